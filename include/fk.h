@@ -1,0 +1,125 @@
+/* fk.h -- C ABI of the B200-native Feynman-Kac exit-time hot path (arXiv 2104.14561).
+ *
+ * The path: for every time step, push each grid node one Euler-Maruyama step to its
+ * tensor-product Gauss-Hermite points (Eq. 11, 21), interpolate the exit
+ * probability there with piecewise cubic Hermite polynomials (Eq. 13-15),
+ * give points that left the box the absorbing value, fold the quadrature weights into the
+ * sparse step operator A_nu = Q Psi^nu (Eq. 24-27), and apply the operators
+ * to all output-time columns in one backward pass (Algorithm 1), which
+ * yields P(t_m, x_j) for every t_m in [0, T_max].
+ *
+ * Every step of that path runs in CUDA kernels for sm_100a inside this library; there is no
+ * CPU fallback.  All entry points return an int code (FK_OK = 0) and never throw.  Unless a
+ * parameter says otherwise the library COPIES what it is given: the caller may free or reuse
+ * its buffers as soon as the call returns.  Device work is ordered on the stream given to
+ * fk_create; calls on one context must not be made concurrently from several threads.
+ *
+ * Index conventions.  d = dimension (1..3); n[k] nodes along dimension k; node index
+ * j = ((i0*n[1])+i1)*n[2]+i2 (last dimension fastest); J = prod n[k].  Steps: dt, N,
+ * T_max = N*dt, t_nu = nu*dt.  Operator nu (0..N-1) uses the coefficients sampled at t_nu
+ * (explicit Euler).  Column m (0..N) is P(t_m, .); column 0 is chi (Eq. 28,
+ * PAPER.md:268); column m = A_0 A_1 ... A_{m-1} chi (Eq. 29).
+ */
+#ifndef FK_B200_H
+#define FK_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fk_ctx fk_ctx; /* opaque; owned by the library; free with fk_destroy */
+
+enum { FK_OK = 0, FK_EINVAL = 1, FK_ENOMEM = 2, FK_ECUDA = 3, FK_ESTATE = 4 };
+
+/* Face rule for a quadrature point that leaves the box through that face (R8/R9):
+ * ABSORB: the point contributes face_value (1 = "exit", the paper's absorbing value); grid
+ *         nodes lying on an ABSORB face are Dirichlet nodes held at face_value.
+ * CLAMP : the point is projected back onto the face and interpolated there; nodes on a CLAMP
+ *         face are updated like interior nodes.
+ * CLAMP dimensions are projected first; among the remaining dimensions that are outside, the
+ * lowest dimension index decides the value. */
+enum { FK_FACE_ABSORB = 0, FK_FACE_CLAMP = 1 };
+
+enum { FK_MEM_HOST = 0, FK_MEM_DEVICE = 1 };
+
+#define FK_ALL_STEPS (-1)
+#define FK_MAX_Q 32
+
+/* Problem statement (PAPER.md:49-51 box and SDE; 117-123 time partition; 134 tensor mesh;
+ * 197-204 Gauss-Hermite rule).  All pointers are HOST pointers read during fk_create only. */
+typedef struct {
+  int d;                   /* 1..3 */
+  int n[3];                /* nodes per dimension, each >= 3 (Eq. 15's end rule needs two
+                              divided differences); unused entries ignored */
+  const double* x[3];      /* x[k][0..n[k]-1], strictly increasing; x[k][0] = alpha_k and
+                              x[k][n[k]-1] = beta_k are the faces of the box; may be
+                              non-uniform */
+  double dt;               /* > 0 */
+  int N;                   /* >= 1 time steps; N+1 output columns */
+  int Q[3];                /* Gauss-Hermite points per dimension, 1..FK_MAX_Q */
+  int face_kind[3][2];     /* [dim][0 = lower face, 1 = upper face] */
+  double face_value[3][2]; /* g of ABSORB faces; ignored for CLAMP */
+  int coeff_slots;         /* number of per-step coefficient slots kept on the device:
+                              N (or 0) = the full table; 1 <= s < N = a ring, step nu lives in
+                              slot nu % s and must be (re)loaded before fk_evolve needs it */
+  int device;              /* CUDA device ordinal */
+  void* stream;            /* cudaStream_t (e.g. from torch); NULL = the legacy default stream */
+} fk_params;
+
+/* Validate, build the Gauss-Hermite tables, allocate device state and fill both P buffers
+ * with chi (Algorithm 1's "P = repmat(chi)").  On failure *out is NULL and the
+ * code says why (FK_EINVAL: bad parameter; FK_ENOMEM: device allocation; FK_ECUDA). */
+int fk_create(const fk_params* p, fk_ctx** out);
+
+/* Drift b and per-dimension noise amplitude sigma (diagonal sigma of Eq. 1)
+ * sampled on the nodes at t_step: b[d][J], sigma[d][J], fp64, in host (mem = FK_MEM_HOST) or
+ * device (FK_MEM_DEVICE, same device) memory.  step in 0..N-1 fills slot step % coeff_slots;
+ * step = FK_ALL_STEPS declares the problem autonomous: the one slice is used by every step.
+ * Values at Dirichlet nodes are never read.  sigma must be >= 0 at updated nodes (not
+ * checked; a negative sigma reverses the order of the quadrature points and is undefined).
+ * Copies are stream-ordered; a host buffer may be reused when the call returns. */
+int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int mem);
+
+/* Same for `count` consecutive steps step0..step0+count-1: b and sigma are [count][d][J].
+ * count must not exceed coeff_slots. */
+int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const double* sigma,
+                        int mem);
+
+/* Algorithm 1's loop for n = n_from, n_from-1, ..., n_to+1: assemble the
+ * operator nu = n-1 once and update columns n..N.  The first call after fk_create/fk_reset
+ * must have n_from = N; later calls continue where the previous one stopped (n_from = its
+ * n_to); after n_to = 0 all columns are final.  Asynchronous: kernels are queued on the
+ * stream.  FK_ESTATE: wrong n_from, or a needed coefficient slot does not hold that step. */
+int fk_evolve(fk_ctx* c, int n_from, int n_to);
+
+/* Refill P with chi and rewind to n = N; coefficient slots are kept. */
+int fk_reset(fk_ctx* c);
+
+/* Copy columns m0..m1-1 out as out[(m1-m0)][J] (row m-m0 = P(t_m, .), node index fastest),
+ * to host or device memory.  Valid for any column once fk_evolve has reached n_to = 0; before
+ * that only column 0 and, after reaching n, nothing else is final (FK_ESTATE).  The call
+ * synchronises the stream when `mem` is FK_MEM_HOST. */
+int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem);
+
+/* Per-kernel-class device time of the fk_evolve calls since the last fk_reset, measured with
+ * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[3] and
+ * launches[3] are indexed FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY.  Synchronises the stream. */
+enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_COUNT = 3 };
+int fk_profile(fk_ctx* c, int on);
+int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
+
+/* Total kernels launched by this context since fk_create (all entry points). */
+long long fk_launch_count(const fk_ctx* c);
+
+void fk_destroy(fk_ctx* c);
+
+/* Text of the last error on this context ("" if none); for a failed fk_create pass NULL. */
+const char* fk_last_error(const fk_ctx* c);
+
+/* Gauss-Hermite rule the library uses (a ascending, weights summing to 1); for inspection. */
+int fk_gauss_hermite(int Q, double* a, double* w);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FK_B200_H */

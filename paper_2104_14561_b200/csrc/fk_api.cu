@@ -1,0 +1,430 @@
+// fk_api.cu -- the C ABI of include/fk.h: validation, Gauss-Hermite tables, device state and
+// the loop of Algorithm 1.  All arithmetic of the path runs in the kernels
+// of fk_kernels.cu; this file only orders them on the caller's stream.
+#include "../../include/fk.h"
+#include "fk_internal.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct EventPair { cudaEvent_t a, b; int cls; };
+
+}  // namespace
+
+struct fk_ctx {
+  FkGrid g;
+  int N = 0, slots = 0, device = 0, n_chunks = 0;
+  cudaStream_t stream = nullptr;
+  double* d_x[3] = {nullptr, nullptr, nullptr};
+  double* d_invh[3] = {nullptr, nullptr, nullptr};
+  double* d_coef = nullptr;            // [slots][2][d][J]: b then sigma per slot
+  std::vector<int> slot_step;          // step held by each slot, -2 = empty
+  bool autonomous = false;
+  double* d_P[2] = {nullptr, nullptr};
+  int cur = 0;                         // buffer holding the current state
+  double* d_dP = nullptr;
+  FkOperator op = {nullptr, nullptr, nullptr, nullptr};
+  double* d_stage = nullptr;           // fk_read staging for host destinations
+  size_t stage_bytes = 0;
+  int n_next = 0;                      // the n the next fk_evolve must start from
+  long long launches = 0;
+  bool profiling = false;
+  std::vector<EventPair> events;
+  std::vector<EventPair> event_pool;
+  std::string err;
+};
+
+namespace {
+
+int fail(fk_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return code;
+}
+
+int cuda_fail(fk_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, e == cudaErrorMemoryAllocation ? FK_ENOMEM : FK_ECUDA,
+              std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define FK_CUDA(c, call)                                       \
+  do {                                                         \
+    cudaError_t e_ = (call);                                   \
+    if (e_ != cudaSuccess) return cuda_fail((c), e_, #call);   \
+  } while (0)
+
+// ------------------------------------------------------------------------------------------
+// Gauss-Hermite rule for the density pi^{-1/2} exp(-xi^2) by Golub-Welsch:
+// the nodes are the eigenvalues of the Jacobi matrix with zero diagonal and off-diagonal
+// sqrt(k/2), found by Sturm-sequence bisection and polished by Newton on the orthonormal
+// polynomial p_Q; the weights are the Christoffel numbers 1 / sum_{k<Q} p_k(a)^2, which sum
+// to 1 for this (normalised) density.
+// ------------------------------------------------------------------------------------------
+void orthonormal_hermite(int Q, long double x, long double* p /*Q+1*/) {
+  p[0] = 1.0L;
+  if (Q >= 1) p[1] = x * std::sqrt(2.0L);
+  for (int k = 1; k < Q; ++k)
+    p[k + 1] = (x * p[k] - std::sqrt(k / 2.0L) * p[k - 1]) / std::sqrt((k + 1) / 2.0L);
+}
+
+int sturm_count(int Q, long double x) {  // eigenvalues of the Jacobi matrix below x
+  int count = 0;
+  long double q = -x;
+  if (q < 0) ++count;
+  for (int k = 1; k < Q; ++k) {
+    long double off2 = k / 2.0L;
+    if (q == 0.0L) q = 1e-300L;
+    q = -x - off2 / q;
+    if (q < 0) ++count;
+  }
+  return count;
+}
+
+void gauss_hermite(int Q, double* a, double* w) {
+  const long double bound = std::sqrt(2.0L * Q + 1.0L) + 1.0L;
+  std::vector<long double> p(Q + 1);
+  for (int i = 0; i < Q; ++i) {
+    long double lo = -bound, hi = bound;
+    for (int it = 0; it < 120; ++it) {
+      long double mid = 0.5L * (lo + hi);
+      if (sturm_count(Q, mid) <= i) lo = mid; else hi = mid;
+    }
+    long double r = 0.5L * (lo + hi);
+    for (int it = 0; it < 3; ++it) {     // p_Q' = sqrt(2Q) p_{Q-1}
+      orthonormal_hermite(Q, r, p.data());
+      r -= p[Q] / (std::sqrt(2.0L * Q) * p[Q - 1]);
+    }
+    if (Q % 2 == 1 && i == Q / 2) r = 0.0L;
+    orthonormal_hermite(Q, r, p.data());
+    long double s = 0.0L;
+    for (int k = 0; k < Q; ++k) s += p[k] * p[k];
+    a[i] = (double)r;
+    w[i] = (double)(1.0L / s);
+  }
+  for (int i = 0; i < Q / 2; ++i) {      // enforce the exact symmetry of the rule
+    double am = 0.5 * (a[Q - 1 - i] - a[i]), wm = 0.5 * (w[i] + w[Q - 1 - i]);
+    a[i] = -am; a[Q - 1 - i] = am;
+    w[i] = wm; w[Q - 1 - i] = wm;
+  }
+}
+
+void release(fk_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  for (int k = 0; k < 3; ++k) { cudaFree(c->d_x[k]); cudaFree(c->d_invh[k]); }
+  cudaFree(c->d_coef);
+  cudaFree(c->d_P[0]);
+  cudaFree(c->d_P[1]);
+  cudaFree(c->d_dP);
+  cudaFree(c->op.w);
+  cudaFree(c->op.off);
+  cudaFree(c->op.cnt);
+  cudaFree(c->op.c);
+  cudaFree(c->d_stage);
+  for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  for (auto& e : c->event_pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  delete c;
+}
+
+}  // namespace
+
+// ==========================================================================================
+// entry points
+// ==========================================================================================
+extern "C" {
+
+int fk_gauss_hermite(int Q, double* a, double* w) {
+  if (Q < 1 || Q > FK_MAX_Q || !a || !w) return FK_EINVAL;
+  gauss_hermite(Q, a, w);
+  return FK_OK;
+}
+
+const char* fk_last_error(const fk_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+long long fk_launch_count(const fk_ctx* c) { return c ? c->launches : 0; }
+
+void fk_destroy(fk_ctx* c) { release(c); }
+
+int fk_create(const fk_params* p, fk_ctx** out) {
+  if (!out) return fail(nullptr, FK_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!p) return fail(nullptr, FK_EINVAL, "params is NULL");
+  if (p->d < 1 || p->d > 3) return fail(nullptr, FK_EINVAL, "d must be 1..3");
+  if (!(p->dt > 0.0) || !std::isfinite(p->dt)) return fail(nullptr, FK_EINVAL, "dt must be > 0");
+  if (p->N < 1) return fail(nullptr, FK_EINVAL, "N must be >= 1");
+  long long J = 1;
+  for (int k = 0; k < p->d; ++k) {
+    if (p->n[k] < 3) return fail(nullptr, FK_EINVAL, "each n[k] must be >= 3");
+    if (!p->x[k]) return fail(nullptr, FK_EINVAL, "x[k] is NULL");
+    if (p->Q[k] < 1 || p->Q[k] > FK_MAX_Q) return fail(nullptr, FK_EINVAL, "Q[k] must be 1..32");
+    for (int i = 0; i < p->n[k]; ++i)
+      if (!std::isfinite(p->x[k][i]) || (i > 0 && !(p->x[k][i] > p->x[k][i - 1])))
+        return fail(nullptr, FK_EINVAL, "x[k] must be finite and strictly increasing");
+    for (int s = 0; s < 2; ++s) {
+      if (p->face_kind[k][s] != FK_FACE_ABSORB && p->face_kind[k][s] != FK_FACE_CLAMP)
+        return fail(nullptr, FK_EINVAL, "unknown face_kind");
+      if (p->face_kind[k][s] == FK_FACE_ABSORB && !std::isfinite(p->face_value[k][s]))
+        return fail(nullptr, FK_EINVAL, "face_value of an ABSORB face must be finite");
+    }
+    J *= p->n[k];
+    if (J * FK_CW >= (1LL << 31)) return fail(nullptr, FK_EINVAL, "grid too large (J*32 must be < 2^31)");
+  }
+  int slots = p->coeff_slots;
+  if (slots < 0 || slots > p->N) return fail(nullptr, FK_EINVAL, "coeff_slots must be 0..N");
+  if (slots == 0) slots = p->N;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(nullptr, FK_ECUDA, "no CUDA device: this library has no CPU path");
+  if (p->device < 0 || p->device >= ndev) return fail(nullptr, FK_EINVAL, "bad device ordinal");
+
+  fk_ctx* c = new (std::nothrow) fk_ctx();
+  if (!c) return fail(nullptr, FK_ENOMEM, "host allocation failed");
+  c->device = p->device;
+  c->stream = (cudaStream_t)p->stream;
+  c->N = p->N;
+  c->slots = slots;
+  c->n_chunks = p->N / FK_CW + 1;          // columns 0..N
+  c->n_next = p->N;
+  c->slot_step.assign(slots, -2);
+
+  FkGrid& g = c->g;
+  std::memset(&g, 0, sizeof(g));
+  g.d = p->d;
+  g.J = J;
+  g.dt = p->dt;
+  g.sq = std::sqrt(2.0 * p->dt);
+  int qoff = 0;
+  for (int k = 0; k < 3; ++k) { g.n[k] = 1; g.Q[k] = 0; g.stride[k] = 0; }
+  long long st = 1;
+  for (int k = p->d - 1; k >= 0; --k) { g.stride[k] = st; st *= p->n[k]; }
+  for (int k = 0; k < p->d; ++k) {
+    g.n[k] = p->n[k];
+    g.Q[k] = p->Q[k];
+    g.qoff[k] = qoff;
+    qoff += 2 * p->Q[k];
+    g.lo[k] = p->x[k][0];
+    g.hi[k] = p->x[k][p->n[k] - 1];
+    g.inv_h0[k] = (p->n[k] - 1) / (g.hi[k] - g.lo[k]);
+    const double h0 = (g.hi[k] - g.lo[k]) / (p->n[k] - 1);
+    int uniform = 1;
+    for (int i = 0; i < p->n[k]; ++i)
+      if (std::fabs(p->x[k][i] - (g.lo[k] + i * h0)) > 1e-9 * h0) uniform = 0;
+    g.uniform[k] = uniform;
+    for (int s = 0; s < 2; ++s) {
+      g.face_kind[k][s] = p->face_kind[k][s];
+      g.face_value[k][s] = p->face_value[k][s];
+    }
+    gauss_hermite(p->Q[k], g.gh_a[k], g.gh_w[k]);
+  }
+  g.RS = qoff;
+
+#define FK_CREATE_CUDA(call)                                                    \
+  do {                                                                          \
+    cudaError_t e_ = (call);                                                    \
+    if (e_ != cudaSuccess) {                                                    \
+      int code_ = cuda_fail(nullptr, e_, #call);                                \
+      release(c);                                                               \
+      return code_;                                                             \
+    }                                                                           \
+  } while (0)
+
+  FK_CREATE_CUDA(cudaSetDevice(c->device));
+  for (int k = 0; k < p->d; ++k) {
+    const int n = p->n[k];
+    std::vector<double> ih(n - 1);
+    for (int i = 0; i < n - 1; ++i) ih[i] = 1.0 / (p->x[k][i + 1] - p->x[k][i]);
+    FK_CREATE_CUDA(cudaMalloc(&c->d_x[k], sizeof(double) * n));
+    FK_CREATE_CUDA(cudaMalloc(&c->d_invh[k], sizeof(double) * (n - 1)));
+    FK_CREATE_CUDA(cudaMemcpyAsync(c->d_x[k], p->x[k], sizeof(double) * n, cudaMemcpyHostToDevice, c->stream));
+    FK_CREATE_CUDA(cudaMemcpyAsync(c->d_invh[k], ih.data(), sizeof(double) * (n - 1), cudaMemcpyHostToDevice, c->stream));
+    FK_CREATE_CUDA(cudaStreamSynchronize(c->stream));   // ih is a local
+    g.x[k] = c->d_x[k];
+    g.inv_h[k] = c->d_invh[k];
+  }
+  const size_t buf = sizeof(double) * (size_t)c->n_chunks * J * FK_CW;
+  FK_CREATE_CUDA(cudaMalloc(&c->d_P[0], buf));
+  FK_CREATE_CUDA(cudaMalloc(&c->d_P[1], buf));
+  FK_CREATE_CUDA(cudaMalloc(&c->d_dP, buf * p->d));
+  FK_CREATE_CUDA(cudaMalloc(&c->d_coef, sizeof(double) * (size_t)slots * 2 * p->d * J));
+  FK_CREATE_CUDA(cudaMalloc(&c->op.w, sizeof(double2) * (size_t)J * g.RS));
+  FK_CREATE_CUDA(cudaMalloc(&c->op.off, sizeof(int) * (size_t)J * g.RS));
+  FK_CREATE_CUDA(cudaMalloc(&c->op.cnt, sizeof(int) * (size_t)J * 4));
+  FK_CREATE_CUDA(cudaMalloc(&c->op.c, sizeof(double) * (size_t)J));
+  FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[0], c->n_chunks, c->stream));
+  FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[1], c->n_chunks, c->stream));
+  c->launches += 2;
+#undef FK_CREATE_CUDA
+  *out = c;
+  return FK_OK;
+}
+
+int fk_reset(fk_ctx* c) {
+  if (!c) return FK_EINVAL;
+  FK_CUDA(c, cudaSetDevice(c->device));
+  FK_CUDA(c, fk_launch_fill_chi(c->g, c->d_P[0], c->n_chunks, c->stream));
+  FK_CUDA(c, fk_launch_fill_chi(c->g, c->d_P[1], c->n_chunks, c->stream));
+  c->launches += 2;
+  c->cur = 0;
+  c->n_next = c->N;
+  for (auto& e : c->events) c->event_pool.push_back(e);
+  c->events.clear();
+  return FK_OK;
+}
+
+int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const double* sigma,
+                        int mem) {
+  if (!c) return FK_EINVAL;
+  if (!b || !sigma) return fail(c, FK_EINVAL, "b or sigma is NULL");
+  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
+  if (count < 1 || count > c->slots) return fail(c, FK_EINVAL, "count must be 1..coeff_slots");
+  if (step0 < 0 || step0 + count > c->N) return fail(c, FK_EINVAL, "step range outside 0..N-1");
+  FK_CUDA(c, cudaSetDevice(c->device));
+  const size_t slice = (size_t)c->g.d * c->g.J;      // doubles per [d][J] array
+  const cudaMemcpyKind kind = mem == FK_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  for (int i = 0; i < count; ++i) {
+    const int step = step0 + i, slot = step % c->slots;
+    double* dst = c->d_coef + (size_t)slot * 2 * slice;
+    FK_CUDA(c, cudaMemcpyAsync(dst, b + (size_t)i * slice, sizeof(double) * slice, kind, c->stream));
+    FK_CUDA(c, cudaMemcpyAsync(dst + slice, sigma + (size_t)i * slice, sizeof(double) * slice, kind, c->stream));
+    c->slot_step[slot] = step;
+  }
+  c->autonomous = false;
+  if (mem == FK_MEM_HOST) FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  return FK_OK;
+}
+
+int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int mem) {
+  if (!c) return FK_EINVAL;
+  if (step != FK_ALL_STEPS) return fk_set_coeffs_range(c, step, 1, b, sigma, mem);
+  if (!b || !sigma) return fail(c, FK_EINVAL, "b or sigma is NULL");
+  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
+  FK_CUDA(c, cudaSetDevice(c->device));
+  const size_t slice = (size_t)c->g.d * c->g.J;
+  const cudaMemcpyKind kind = mem == FK_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  FK_CUDA(c, cudaMemcpyAsync(c->d_coef, b, sizeof(double) * slice, kind, c->stream));
+  FK_CUDA(c, cudaMemcpyAsync(c->d_coef + slice, sigma, sizeof(double) * slice, kind, c->stream));
+  std::fill(c->slot_step.begin(), c->slot_step.end(), -2);
+  c->autonomous = true;
+  if (mem == FK_MEM_HOST) FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  return FK_OK;
+}
+
+
+// one kernel launch, optionally bracketed by a pair of events of class `cls`
+#define FK_LAUNCH(c, cls_, call)                                                       \
+  do {                                                                                 \
+    EventPair ep_{};                                                                   \
+    if ((c)->profiling) {                                                              \
+      if (!(c)->event_pool.empty()) { ep_ = (c)->event_pool.back(); (c)->event_pool.pop_back(); } \
+      else { FK_CUDA(c, cudaEventCreate(&ep_.a)); FK_CUDA(c, cudaEventCreate(&ep_.b)); } \
+      ep_.cls = (cls_);                                                                \
+      FK_CUDA(c, cudaEventRecord(ep_.a, (c)->stream));                                 \
+    }                                                                                  \
+    FK_CUDA(c, call);                                                                  \
+    ++(c)->launches;                                                                   \
+    if ((c)->profiling) {                                                              \
+      FK_CUDA(c, cudaEventRecord(ep_.b, (c)->stream));                                 \
+      (c)->events.push_back(ep_);                                                      \
+    }                                                                                  \
+  } while (0)
+
+int fk_evolve(fk_ctx* c, int n_from, int n_to) {
+  if (!c) return FK_EINVAL;
+  if (n_from != c->n_next) return fail(c, FK_ESTATE, "n_from must continue where the last fk_evolve stopped (N after create/reset)");
+  if (n_to < 0 || n_to > n_from) return fail(c, FK_EINVAL, "need 0 <= n_to <= n_from");
+  FK_CUDA(c, cudaSetDevice(c->device));
+  const size_t slice = (size_t)c->g.d * c->g.J;
+  const int last_chunk = c->N / FK_CW + 1;             // one past the chunk of column N
+  for (int n = n_from; n > n_to; --n) {
+    const int nu = n - 1;
+    int slot = 0;
+    if (!c->autonomous) {
+      slot = nu % c->slots;
+      if (c->slot_step[slot] != nu) {
+        c->n_next = n;
+        char msg[96];
+        std::snprintf(msg, sizeof msg, "coefficients of step %d are not loaded", nu);
+        return fail(c, FK_ESTATE, msg);
+      }
+    }
+    const double* b = c->d_coef + (size_t)slot * 2 * slice;
+    const int chunk0 = n / FK_CW;                      // first chunk with an active column
+    const double* Pold = c->d_P[c->cur];
+    double* Pnew = c->d_P[c->cur ^ 1];
+    FK_LAUNCH(c, FK_K_ASSEMBLE, fk_launch_assemble(c->g, b, b + slice, c->op, c->stream));
+    FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, c->stream));
+    FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, c->stream));
+    c->cur ^= 1;
+    c->n_next = n - 1;
+  }
+  return FK_OK;
+}
+
+int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem) {
+  if (!c) return FK_EINVAL;
+  if (!out) return fail(c, FK_EINVAL, "out is NULL");
+  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
+  if (m0 < 0 || m1 > c->N + 1 || m0 >= m1) return fail(c, FK_EINVAL, "need 0 <= m0 < m1 <= N+1");
+  if (c->n_next != 0 && m1 > 1) return fail(c, FK_ESTATE, "columns other than 0 are final only after fk_evolve reached n_to = 0");
+  FK_CUDA(c, cudaSetDevice(c->device));
+  const double* P = c->d_P[c->cur];
+  const size_t col = sizeof(double) * (size_t)c->g.J;
+  if (mem == FK_MEM_DEVICE) {
+    FK_CUDA(c, fk_launch_gather_columns(c->g, P, m0, m1, out, c->stream));
+    ++c->launches;
+    return FK_OK;
+  }
+  // host destination: gather into a bounded device staging buffer, copy out batch by batch
+  const size_t want = (size_t)256 << 20;
+  int batch = (int)(want / col);
+  if (batch < FK_CW) batch = FK_CW;
+  batch -= batch % FK_CW;
+  if (batch > m1 - m0) batch = m1 - m0;
+  if (c->stage_bytes < (size_t)batch * col) {
+    cudaFree(c->d_stage);
+    c->d_stage = nullptr;
+    c->stage_bytes = 0;
+    FK_CUDA(c, cudaMalloc(&c->d_stage, (size_t)batch * col));
+    c->stage_bytes = (size_t)batch * col;
+  }
+  for (int a = m0; a < m1; a += batch) {
+    const int e = a + batch < m1 ? a + batch : m1;
+    FK_CUDA(c, fk_launch_gather_columns(c->g, P, a, e, c->d_stage, c->stream));
+    ++c->launches;
+    FK_CUDA(c, cudaMemcpyAsync(out + (size_t)(a - m0) * c->g.J, c->d_stage, (size_t)(e - a) * col,
+                               cudaMemcpyDeviceToHost, c->stream));
+    FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return FK_OK;
+}
+
+int fk_profile(fk_ctx* c, int on) {
+  if (!c) return FK_EINVAL;
+  c->profiling = on != 0;
+  return FK_OK;
+}
+
+int fk_profile_read(fk_ctx* c, double* ms, long long* launches) {
+  if (!c) return FK_EINVAL;
+  if (!ms || !launches) return fail(c, FK_EINVAL, "ms or launches is NULL");
+  FK_CUDA(c, cudaSetDevice(c->device));
+  FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < FK_K_COUNT; ++k) { ms[k] = 0.0; launches[k] = 0; }
+  for (auto& e : c->events) {
+    float t = 0.f;
+    FK_CUDA(c, cudaEventElapsedTime(&t, e.a, e.b));
+    ms[e.cls] += t;
+    ++launches[e.cls];
+  }
+  return FK_OK;
+}
+
+}  // extern "C"

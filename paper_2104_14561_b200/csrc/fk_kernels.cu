@@ -1,0 +1,361 @@
+// fk_kernels.cu -- sm_100a kernels of the Feynman-Kac exit-time hot path (arXiv 2104.14561).
+//
+//   fk_fill_chi      Eq. 28 / Algorithm 1 "P = repmat(chi)"
+//   fk_assemble      Scheme 1 step 1 + the quadrature fold: one row of A_nu = Q Psi^nu per
+//                    node, in factored form (Eq. 21, 147 Eq. 14, 256-264)
+//   fk_slopes        F: the PCHIP nodal slopes of Eq. 15 for every active column
+//
+//   fk_apply         P(:, n:N) <- A_nu [P; dP](:, n:N)
+//   fk_gather        read-out of columns into [m][J] order
+//
+// Thread mapping of the two hot kernels: lane = output-time column inside a 32-column chunk,
+// warp = one node.  Every P / dP access of a warp is one aligned 256-byte row whatever the
+// shape of the stencil (scattered 1-D rows with Q = 16, clamped rows that reach across the
+// whole box, ...), and the operator row is warp-uniform, so it is fetched by broadcast loads.
+#include "fk_internal.h"
+
+namespace {
+
+__device__ __forceinline__ void unravel(const FkGrid& g, long long j, int idx[3]) {
+  idx[0] = idx[1] = idx[2] = 0;
+  for (int k = g.d - 1; k >= 0; --k) {
+    long long q = j / g.n[k];
+    idx[k] = (int)(j - q * g.n[k]);
+    j = q;
+  }
+}
+
+// node on an ABSORB face?  lowest dimension decides the value (R9)
+__device__ __forceinline__ bool dirichlet(const FkGrid& g, const int idx[3], double* val) {
+  for (int k = 0; k < g.d; ++k) {
+    if (idx[k] == 0 && g.face_kind[k][0] == 0) { *val = g.face_value[k][0]; return true; }
+    if (idx[k] == g.n[k] - 1 && g.face_kind[k][1] == 0) { *val = g.face_value[k][1]; return true; }
+  }
+  return false;
+}
+
+// ------------------------------------------------------------------------------------------
+// chi into every lane of every chunk (also the padding columns beyond N)
+// ------------------------------------------------------------------------------------------
+__global__ void fk_fill_chi(FkGrid g, double* __restrict__ P, int n_chunks) {
+  long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
+  if (j >= g.J) return;
+  int idx[3];
+  unravel(g, j, idx);
+  double v;
+  if (!dirichlet(g, idx, &v)) v = 0.0;
+  for (int c = blockIdx.y; c < n_chunks; c += gridDim.y)
+    P[((size_t)c * g.J + j) * FK_CW + threadIdx.x] = v;
+}
+
+// ------------------------------------------------------------------------------------------
+// cell c with x[c] <= z < x[c+1], 0 <= c <= n-2 (z == x[n-1] falls in the last cell); z is
+// inside [lo, hi] here.  The index is clamped whatever z is, so a NaN coefficient can only
+// produce NaN values, never an out-of-range access.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int locate(const FkGrid& g, int k, double z) {
+  const double* __restrict__ x = g.x[k];
+  const int n = g.n[k];
+  int c;
+  if (g.uniform[k]) {
+    c = __double2int_rd((z - g.lo[k]) * g.inv_h0[k]);
+    c = max(0, min(c, n - 2));
+    while (c > 0 && z < x[c]) --c;
+    while (c < n - 2 && z >= x[c + 1]) ++c;
+  } else {
+    int lo = 0, hi = n - 1;                 // invariant: x[lo] <= z (or lo == 0), z < x[hi] (or hi == n-1)
+    while (hi - lo > 1) {
+      int mid = (lo + hi) >> 1;
+      if (z >= x[mid]) lo = mid; else hi = mid;
+    }
+    c = min(lo, n - 2);
+  }
+  return c;
+}
+
+// ------------------------------------------------------------------------------------------
+// fk_assemble: one thread per node.  For each dimension k the Q_k points
+//   z_q = (x + b dt) + (sigma sqrt(2 dt)) a_q          (Eq. 21; products and sums NOT fused,
+//                                                       so cells agree with any fp64 reading)
+// are visited in ascending order (sigma >= 0), so their cells are non-decreasing and the
+// weights w_q * {Hermite basis of Eq. 14} can be merged onto distinct nodes with a two-entry
+// window that is flushed to the row as it moves.  Points outside an ABSORB face add
+// w_q * g to e_k; CLAMP faces project the point.  With m_k the inside mass of dimension k,
+//   c_j = sum_k (prod_{l<k} m_l) e_k                   (lowest outside dimension decides, R9).
+// ------------------------------------------------------------------------------------------
+__global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
+                            const double* __restrict__ sigma, FkOperator op) {
+  long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= g.J) return;
+  int idx[3];
+  unravel(g, j, idx);
+  int* cnt = op.cnt + j * 4;
+  double gval;
+  if (dirichlet(g, idx, &gval)) {
+    cnt[0] = cnt[1] = cnt[2] = 0;
+    cnt[3] = 1;
+    op.c[j] = gval;
+    return;
+  }
+  double2* __restrict__ roww = op.w + (size_t)j * g.RS;
+  int* __restrict__ rowo = op.off + (size_t)j * g.RS;
+  double cj = 0.0, mass = 1.0;
+  for (int k = 0; k < g.d; ++k) {
+    const double xk = g.x[k][idx[k]];
+    const double centre = __dadd_rn(xk, __dmul_rn(b[(size_t)k * g.J + j], g.dt));
+    const double spread = __dmul_rn(sigma[(size_t)k * g.J + j], g.sq);
+    const double lo = g.lo[k], hi = g.hi[k];
+    const long long unit = g.stride[k] * FK_CW;
+    double ek = 0.0, mk = 0.0;
+    int count = 0;
+    int cprev = -2;
+    double aL = 0.0, bL = 0.0, aR = 0.0, bR = 0.0;
+    double2* wk = roww + g.qoff[k];
+    int* ok = rowo + g.qoff[k];
+    for (int q = 0; q < g.Q[k]; ++q) {
+      double z = __dadd_rn(centre, __dmul_rn(spread, g.gh_a[k][q]));
+      const double w = g.gh_w[k][q];
+      if (z < lo) {
+        if (g.face_kind[k][0] == 1) z = lo; else { ek += w * g.face_value[k][0]; continue; }
+      } else if (z > hi) {
+        if (g.face_kind[k][1] == 1) z = hi; else { ek += w * g.face_value[k][1]; continue; }
+      }
+      mk += w;
+      const int c = locate(g, k, z);
+      const double h = g.x[k][c + 1] - g.x[k][c];
+      const double t = (z - g.x[k][c]) * g.inv_h[k][c];
+      const double u = 1.0 - t;
+      // Eq. 14 with t = s/h: value-left (1+2t)(1-t)^2, value-right t^2(3-2t),
+      // slope-left h t(1-t)^2, slope-right h t^2(t-1)
+      const double vL = w * ((1.0 + 2.0 * t) * u * u);
+      const double vR = w * (t * t * (3.0 - 2.0 * t));
+      const double sL = w * (h * t * u * u);
+      const double sR = w * (h * t * t * (t - 1.0));
+      if (c == cprev) {
+        aL += vL; bL += sL; aR += vR; bR += sR;
+      } else if (c == cprev + 1) {
+        wk[count] = make_double2(aL, bL); ok[count] = (int)(cprev * unit); ++count;
+        aL = aR + vL; bL = bR + sL; aR = vR; bR = sR;
+        cprev = c;
+      } else {
+        if (cprev >= 0) {
+          wk[count] = make_double2(aL, bL); ok[count] = (int)(cprev * unit); ++count;
+          wk[count] = make_double2(aR, bR); ok[count] = (int)((cprev + 1) * unit); ++count;
+        }
+        aL = vL; bL = sL; aR = vR; bR = sR;
+        cprev = c;
+      }
+    }
+    if (cprev >= 0) {
+      wk[count] = make_double2(aL, bL); ok[count] = (int)(cprev * unit); ++count;
+      wk[count] = make_double2(aR, bR); ok[count] = (int)((cprev + 1) * unit); ++count;
+    }
+    cnt[k] = count;
+    cj += mass * ek;
+    mass *= mk;
+  }
+  for (int k = g.d; k < 3; ++k) cnt[k] = 0;
+  cnt[3] = 0;
+  op.c[j] = cj;
+}
+
+
+// ------------------------------------------------------------------------------------------
+// Eq. 15: 0 if the two divided differences differ in sign or one is 0 (R7), else their
+// harmonic mean 2ab/(a+b) (same-sign operands: the sum does not cancel).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double harmonic(double a, double b) {
+  const bool same = (a > 0.0 && b > 0.0) || (a < 0.0 && b < 0.0);
+  return same ? (2.0 * a * b) / (a + b) : 0.0;
+}
+
+// ------------------------------------------------------------------------------------------
+// fk_slopes: block (32, 8): lane = column, threadIdx.y = node; grid.y = active chunks.
+// dP_k(j) from the grid line of axis k through j; end nodes use the first / last two
+// divided differences (R6).
+// ------------------------------------------------------------------------------------------
+__global__ void fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP,
+                          int n_chunks, int chunk0) {
+  long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
+  if (j >= g.J) return;
+  const int c = chunk0 + blockIdx.y;
+  int idx[3];
+  unravel(g, j, idx);
+  const size_t chunk_elems = (size_t)g.J * FK_CW;
+  const double* __restrict__ u = P + (size_t)c * chunk_elems + (size_t)j * FK_CW + threadIdx.x;
+  const double u0 = u[0];
+  for (int k = 0; k < g.d; ++k) {
+    const long long s = g.stride[k] * FK_CW;
+    const int i = idx[k], n = g.n[k];
+    const double* __restrict__ ih = g.inv_h[k];
+    double da, db;
+    if (i == 0) {
+      const double u1 = u[s], u2 = u[2 * s];
+      da = (u1 - u0) * ih[0];
+      db = (u2 - u1) * ih[1];
+    } else if (i == n - 1) {
+      const double u1 = u[-s], u2 = u[-2 * s];
+      da = (u0 - u1) * ih[n - 2];
+      db = (u1 - u2) * ih[n - 3];
+    } else {
+      da = (u0 - u[-s]) * ih[i - 1];
+      db = (u[s] - u0) * ih[i];
+    }
+    dP[((size_t)k * n_chunks + c) * chunk_elems + (size_t)j * FK_CW + threadIdx.x] =
+        harmonic(da, db);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// fk_apply<D>: block (32, 8), lane = column, threadIdx.y = node; grid.y = active chunks.
+//   out = c_j + sum_{i0} [ alpha0 A'(i0) + beta0 B0'(i0) ]
+//   A'(i0)  = sum_{i1} [ alpha1 A(i0,i1) + beta1 B1(i0,i1) ],  B0'(i0) = sum_{i1} alpha1 B0(i0,i1)
+//   A(i0,i1)  = sum_{i2} [ alpha2 u + beta2 du2 ],  Bk(i0,i1) = sum_{i2} alpha2 du_k
+// i.e. Eq. 13 with the quadrature weights folded in, contracted one dimension at a time.
+// Lanes whose column is not active (m < n: still chi; m > N: padding) compute and discard.
+// ------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(256)
+fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
+         const double* __restrict__ dP, double* __restrict__ Pnew, int n_chunks, int chunk0,
+         int n, int N) {
+  long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
+  if (j >= g.J) return;
+  const int c = chunk0 + blockIdx.y;
+  const int m = c * FK_CW + threadIdx.x;
+  const size_t chunk_elems = (size_t)g.J * FK_CW;
+  const double* __restrict__ u = Pold + (size_t)c * chunk_elems + threadIdx.x;
+  const double* __restrict__ d0 = dP + (size_t)c * chunk_elems + threadIdx.x;
+  const double* __restrict__ d1 = d0 + (size_t)n_chunks * chunk_elems;
+  const double* __restrict__ d2 = d1 + (size_t)n_chunks * chunk_elems;
+  const double2* __restrict__ w = op.w + (size_t)j * g.RS;
+  const int* __restrict__ off = op.off + (size_t)j * g.RS;
+  const int4 cnt = *reinterpret_cast<const int4*>(op.cnt + j * 4);
+  double acc = op.c[j];
+  if (D == 1) {
+    double a0 = 0.0, a1 = 0.0;
+    for (int e = 0; e < cnt.x; ++e) {
+      const double2 w0 = w[e];
+      const int o = off[e];
+      a0 = fma(w0.x, u[o], a0);
+      a1 = fma(w0.y, d0[o], a1);
+    }
+    acc += a0 + a1;
+  } else if (D == 2) {
+    const double2* __restrict__ w1p = w + g.qoff[1];
+    const int* __restrict__ o1p = off + g.qoff[1];
+    for (int e0 = 0; e0 < cnt.x; ++e0) {
+      const double2 w0 = w[e0];
+      const int o0 = off[e0];
+      double A = 0.0, A2 = 0.0, B0 = 0.0;
+      for (int e1 = 0; e1 < cnt.y; ++e1) {
+        const double2 w1 = w1p[e1];
+        const int o = o0 + o1p[e1];
+        A = fma(w1.x, u[o], A);
+        A2 = fma(w1.y, d1[o], A2);
+        B0 = fma(w1.x, d0[o], B0);
+      }
+      acc = fma(w0.x, A + A2, acc);
+      acc = fma(w0.y, B0, acc);
+    }
+  } else {
+    const double2* __restrict__ w1p = w + g.qoff[1];
+    const int* __restrict__ o1p = off + g.qoff[1];
+    const double2* __restrict__ w2p = w + g.qoff[2];
+    const int* __restrict__ o2p = off + g.qoff[2];
+    for (int e0 = 0; e0 < cnt.x; ++e0) {
+      const double2 w0 = w[e0];
+      const int o0 = off[e0];
+      double Ap = 0.0, B0p = 0.0;
+      for (int e1 = 0; e1 < cnt.y; ++e1) {
+        const double2 w1 = w1p[e1];
+        const int o01 = o0 + o1p[e1];
+        double A = 0.0, A2 = 0.0, B0 = 0.0, B1 = 0.0;
+        for (int e2 = 0; e2 < cnt.z; ++e2) {
+          const double2 w2 = w2p[e2];
+          const int o = o01 + o2p[e2];
+          A = fma(w2.x, u[o], A);
+          A2 = fma(w2.y, d2[o], A2);
+          B0 = fma(w2.x, d0[o], B0);
+          B1 = fma(w2.x, d1[o], B1);
+        }
+        Ap = fma(w1.x, A + A2, Ap);
+        Ap = fma(w1.y, B1, Ap);
+        B0p = fma(w1.x, B0, B0p);
+      }
+      acc = fma(w0.x, Ap, acc);
+      acc = fma(w0.y, B0p, acc);
+    }
+  }
+  if (m >= n && m <= N) Pnew[(size_t)c * chunk_elems + (size_t)j * FK_CW + threadIdx.x] = acc;
+}
+
+// ------------------------------------------------------------------------------------------
+// fk_gather: out[m - m0][j] = P[m / 32][j][m % 32]; 32 x 32 transpose through shared memory
+// so that both sides are coalesced.  grid = (node tiles, chunks touched by [m0, m1)).
+// ------------------------------------------------------------------------------------------
+__global__ void fk_gather(FkGrid g, const double* __restrict__ P, int m0, int m1,
+                          double* __restrict__ out) {
+  __shared__ double tile[32][33];
+  const int c = m0 / FK_CW + blockIdx.y;
+  const long long j0 = (long long)blockIdx.x * 32;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    long long j = j0 + r;
+    if (j < g.J) tile[r][threadIdx.x] = P[((size_t)c * g.J + j) * FK_CW + threadIdx.x];
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int m = c * FK_CW + r;
+    long long j = j0 + threadIdx.x;
+    if (m >= m0 && m < m1 && j < g.J) out[(size_t)(m - m0) * g.J + j] = tile[threadIdx.x][r];
+  }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------
+static inline unsigned node_blocks(const FkGrid& g, int per_block) {
+  return (unsigned)((g.J + per_block - 1) / per_block);
+}
+
+cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStream_t s) {
+  dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(n_chunks < 64 ? n_chunks : 64));
+  fk_fill_chi<<<grid, block, 0, s>>>(g, P, n_chunks);
+  return cudaGetLastError();
+}
+
+cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
+                               FkOperator op, cudaStream_t s) {
+  fk_assemble<<<node_blocks(g, 128), 128, 0, s>>>(g, b, sigma, op);
+  return cudaGetLastError();
+}
+
+cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
+                             int chunk0, int chunk1, cudaStream_t s) {
+  dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(chunk1 - chunk0));
+  fk_slopes<<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0);
+  return cudaGetLastError();
+}
+
+cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
+                            double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
+                            cudaStream_t s) {
+  dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(chunk1 - chunk0));
+  if (g.d == 1)
+    fk_apply<1><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N);
+  else if (g.d == 2)
+    fk_apply<2><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N);
+  else
+    fk_apply<3><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N);
+  return cudaGetLastError();
+}
+
+cudaError_t fk_launch_gather_columns(const FkGrid& g, const double* P, int m0, int m1,
+                                     double* out, cudaStream_t s) {
+  const int c0 = m0 / FK_CW, c1 = (m1 - 1) / FK_CW + 1;
+  dim3 block(32, 8), grid(node_blocks(g, 32), (unsigned)(c1 - c0));
+  fk_gather<<<grid, block, 0, s>>>(g, P, m0, m1, out);
+  return cudaGetLastError();
+}

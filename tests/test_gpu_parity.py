@@ -1,0 +1,149 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): max abs error <= 1e-11 in fp64 on the same seeded inputs.
+The reduced shapes of `workloads.small` keep each configuration's structure (faces, Q,
+coefficient formulas, the paper's dt) at sizes the oracle finishes in seconds; they span
+several 8-node blocks and 32-column chunks with ragged tails in both.
+"""
+import numpy as np
+import pytest
+
+from paper_2104_14561_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def fk():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2104_14561_b200 import binding, solve
+    binding.lib()
+    return binding, solve
+
+
+@pytest.fixture(scope="module")
+def oracle_P(oracle_mod):
+    cache = {}
+
+    def get(idx):
+        if idx not in cache:
+            wl = W.small(idx)
+            cache[idx] = (wl, oracle_mod.Oracle(wl).algorithm1())
+        return cache[idx]
+    return get
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_small_config_matches_oracle(fk, oracle_P, idx):
+    _, solve = fk
+    wl, ref = oracle_P(idx)
+    got = solve.evolve(wl)
+    assert got.shape == ref.shape
+    err = np.abs(got - ref).max()
+    assert err <= TOL, f"config {idx}: max abs error {err:.3e}"
+    # column 0 is chi, untouched
+    assert np.array_equal(got[0], ref[0])
+
+
+@pytest.mark.parametrize("idx,slots", [(2, 7), (3, 1), (5, 4)])
+def test_coefficient_ring_equals_full_table(fk, oracle_P, idx, slots):
+    _, solve = fk
+    wl, ref = oracle_P(idx)
+    got = solve.evolve(wl, coeff_slots=slots)
+    assert np.abs(got - ref).max() <= TOL
+
+
+def test_read_subrange_and_device_destination(fk, oracle_P):
+    import torch
+    B, solve = fk
+    wl, ref = oracle_P(3)
+    ctx = solve.create_for(wl, wl.N)
+    try:
+        solve.evolve_loaded(ctx, wl, wl.N)
+        host = np.empty((5, wl.J))
+        B.fk_read(ctx, 30, 35, host)                     # crosses the chunk boundary at 32
+        assert np.abs(host - ref[30:35]).max() <= TOL
+        dev = torch.empty((wl.N + 1, wl.J), dtype=torch.float64, device="cuda")
+        B.fk_read(ctx, 0, wl.N + 1, dev)
+        torch.cuda.synchronize()
+        assert np.abs(dev.cpu().numpy() - ref).max() <= TOL
+        one = np.empty((1, wl.J))
+        B.fk_read(ctx, wl.N, wl.N + 1, one)
+        assert np.abs(one[0] - ref[wl.N]).max() <= TOL
+    finally:
+        B.fk_destroy(ctx)
+
+
+def test_device_coefficients_and_reset(fk, oracle_P):
+    import torch
+    B, solve = fk
+    wl, ref = oracle_P(4)
+    b, s = wl.coeff_table(0, wl.N)
+    tb = torch.from_numpy(b).cuda()
+    ts = torch.from_numpy(s).cuda()
+    stream = torch.cuda.Stream()
+    ctx = solve.create_for(wl, wl.N, stream=stream.cuda_stream)
+    try:
+        for _ in range(2):                                # second pass after fk_reset
+            B.fk_set_coeffs_range(ctx, 0, wl.N, tb, ts)
+            B.fk_evolve(ctx, wl.N, 0)
+            out = np.empty((wl.N + 1, wl.J))
+            B.fk_read(ctx, 0, wl.N + 1, out)
+            assert np.abs(out - ref).max() <= TOL
+            B.fk_reset(ctx)
+    finally:
+        B.fk_destroy(ctx)
+
+
+def test_evolve_in_pieces_equals_one_call(fk, oracle_P):
+    B, solve = fk
+    wl, ref = oracle_P(2)
+    ctx = solve.create_for(wl, wl.N)
+    try:
+        b, s = wl.coeff_table(0, wl.N)
+        B.fk_set_coeffs_range(ctx, 0, wl.N, b, s)
+        B.fk_evolve(ctx, wl.N, 33)
+        B.fk_evolve(ctx, 33, 32)
+        B.fk_evolve(ctx, 32, 0)
+        out = np.empty((wl.N + 1, wl.J))
+        B.fk_read(ctx, 0, wl.N + 1, out)
+        assert np.abs(out - ref).max() <= TOL
+    finally:
+        B.fk_destroy(ctx)
+
+
+def test_state_errors(fk):
+    B, solve = fk
+    wl = W.small(2)
+    ctx = solve.create_for(wl, 4)
+    try:
+        with pytest.raises(B.FkError) as e:
+            B.fk_evolve(ctx, wl.N - 1, 0)                 # must start at N
+        assert e.value.code == B.FK_ESTATE
+        with pytest.raises(B.FkError) as e:
+            B.fk_evolve(ctx, wl.N, 0)                     # nothing loaded
+        assert e.value.code == B.FK_ESTATE
+        out = np.empty((2, wl.J))
+        with pytest.raises(B.FkError) as e:
+            B.fk_read(ctx, 0, 2, out)                     # column 1 not final yet
+        assert e.value.code == B.FK_ESTATE
+        B.fk_read(ctx, 0, 1, out[:1])                     # chi is always readable
+        b, s = wl.coeff_table(0, 5)
+        with pytest.raises(B.FkError) as e:
+            B.fk_set_coeffs_range(ctx, 0, 5, b, s)        # more steps than slots
+        assert e.value.code == B.FK_EINVAL
+    finally:
+        B.fk_destroy(ctx)
+
+
+def test_operator_identities_on_gpu(fk):
+    """u = 1 is reproduced; a Dirichlet value g != 1 is carried (face values, CLAMP faces)."""
+    B, solve = fk
+    wl = W.small(5)
+    got = solve.evolve(wl)
+    assert got.min() >= -1e-12 and got.max() <= 1.0 + 1e-12
+    # P non-decreasing in t to rounding
+    assert (np.diff(got, axis=0) >= -1e-12).all()
