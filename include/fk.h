@@ -102,9 +102,11 @@ int fk_reset(fk_ctx* c);
 int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem);
 
 /* Per-kernel-class device time of the fk_evolve calls since the last fk_reset, measured with
- * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[3] and
- * launches[3] are indexed FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY.  Synchronises the stream. */
-enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_COUNT = 3 };
+ * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[FK_K_COUNT]
+ * and launches[FK_K_COUNT] are indexed FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY (the generic
+ * slopes / apply pair) and FK_K_FUSED (the fused 2-D slopes+apply kernel).  Synchronises the
+ * stream. */
+enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_FUSED = 3, FK_K_COUNT = 4 };
 int fk_profile(fk_ctx* c, int on);
 int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
 

@@ -18,8 +18,8 @@ FK_FACE_ABSORB, FK_FACE_CLAMP = 0, 1
 FK_MEM_HOST, FK_MEM_DEVICE = 0, 1
 FK_ALL_STEPS = -1
 FK_MAX_Q = 32
-FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_COUNT = 0, 1, 2, 3
-KERNEL_CLASSES = ("assemble", "slopes", "apply")
+FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_COUNT = 0, 1, 2, 3, 4
+KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused")
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 
@@ -168,7 +168,7 @@ def fk_profile(ctx, on):
 
 
 def fk_profile_read(ctx):
-    """-> {class: (ms, launches)} for the kernel classes assemble / slopes / apply."""
+    """-> {class: (ms, launches)} for the kernel classes assemble / slopes / apply / fused."""
     ms = (C.c_double * FK_K_COUNT)()
     ln = (C.c_longlong * FK_K_COUNT)()
     _check(ctx, lib().fk_profile_read(ctx, ms, ln))

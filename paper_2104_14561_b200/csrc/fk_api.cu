@@ -31,7 +31,11 @@ struct fk_ctx {
   double* d_P[2] = {nullptr, nullptr};
   int cur = 0;                         // buffer holding the current state
   double* d_dP = nullptr;
-  FkOperator op = {nullptr, nullptr, nullptr, nullptr};
+  FkOperator op = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
+  std::vector<int> h_far;              // host copy, valid when far_valid
+  bool far_valid = false;
+  int sm_count = 148;
   double* d_stage = nullptr;           // fk_read staging for host destinations
   size_t stage_bytes = 0;
   int n_next = 0;                      // the n the next fk_evolve must start from
@@ -127,6 +131,8 @@ void release(fk_ctx* c) {
   cudaFree(c->op.off);
   cudaFree(c->op.cnt);
   cudaFree(c->op.c);
+  cudaFree(c->op.rec);
+  cudaFree(c->d_far);
   cudaFree(c->d_stage);
   for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   for (auto& e : c->event_pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -258,6 +264,14 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   FK_CREATE_CUDA(cudaMalloc(&c->op.off, sizeof(int) * (size_t)J * g.RS));
   FK_CREATE_CUDA(cudaMalloc(&c->op.cnt, sizeof(int) * (size_t)J * 4));
   FK_CREATE_CUDA(cudaMalloc(&c->op.c, sizeof(double) * (size_t)J));
+  FK_CREATE_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
+  if (p->d == 2) {                       // the fused 2-D kernel's records and step classification
+    FK_CREATE_CUDA(cudaMalloc(&c->op.rec, sizeof(FkRec2) * (size_t)J));
+    FK_CREATE_CUDA(cudaMalloc(&c->d_far, sizeof(int) * (size_t)slots));
+    FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots, c->stream));
+    FK_CREATE_CUDA(fk_fused2d_setup());
+    c->h_far.assign(slots, 0);
+  }
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[0], c->n_chunks, c->stream));
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[1], c->n_chunks, c->stream));
   c->launches += 2;
@@ -297,6 +311,16 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
     c->slot_step[slot] = step;
   }
   c->autonomous = false;
+  if (c->g.d == 2) {                     // which of these steps have rows outside the fused halo
+    const int s0 = step0 % c->slots;
+    const int first = count < c->slots - s0 ? count : c->slots - s0;
+    FK_CUDA(c, cudaMemsetAsync(c->d_far + s0, 0, sizeof(int) * (size_t)first, c->stream));
+    if (count > first)
+      FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)(count - first), c->stream));
+    FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, step0, count, c->d_far, c->stream));
+    ++c->launches;
+    c->far_valid = false;
+  }
   if (mem == FK_MEM_HOST) FK_CUDA(c, cudaStreamSynchronize(c->stream));
   return FK_OK;
 }
@@ -313,6 +337,12 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   FK_CUDA(c, cudaMemcpyAsync(c->d_coef + slice, sigma, sizeof(double) * slice, kind, c->stream));
   std::fill(c->slot_step.begin(), c->slot_step.end(), -2);
   c->autonomous = true;
+  if (c->g.d == 2) {
+    FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int), c->stream));
+    FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, 0, 1, c->d_far, c->stream));
+    ++c->launches;
+    c->far_valid = false;
+  }
   if (mem == FK_MEM_HOST) FK_CUDA(c, cudaStreamSynchronize(c->stream));
   return FK_OK;
 }
@@ -343,6 +373,12 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   FK_CUDA(c, cudaSetDevice(c->device));
   const size_t slice = (size_t)c->g.d * c->g.J;
   const int last_chunk = c->N / FK_CW + 1;             // one past the chunk of column N
+  if (c->g.d == 2 && !c->far_valid && n_from > n_to) { // one small read-back per coefficient load
+    FK_CUDA(c, cudaMemcpyAsync(c->h_far.data(), c->d_far, sizeof(int) * (size_t)c->slots,
+                               cudaMemcpyDeviceToHost, c->stream));
+    FK_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->far_valid = true;
+  }
   for (int n = n_from; n > n_to; --n) {
     const int nu = n - 1;
     int slot = 0;
@@ -360,8 +396,14 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
     const double* Pold = c->d_P[c->cur];
     double* Pnew = c->d_P[c->cur ^ 1];
     FK_LAUNCH(c, FK_K_ASSEMBLE, fk_launch_assemble(c->g, b, b + slice, c->op, c->stream));
-    FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, c->stream));
-    FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, c->stream));
+    const bool fused = c->g.d == 2;
+    const bool generic = !fused || c->h_far[slot] > 0;   // rows the fused kernel leaves out
+    if (fused)
+      FK_LAUNCH(c, FK_K_FUSED, fk_launch_fused2d(c->g, c->op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
+    if (generic) {
+      FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, c->stream));
+      FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, c->stream));
+    }
     c->cur ^= 1;
     c->n_next = n - 1;
   }

@@ -1,0 +1,96 @@
+// fk_device.cuh -- device helpers shared by the kernels of the CUDA path (not by oracle/).
+#ifndef FK_DEVICE_CUH
+#define FK_DEVICE_CUH
+
+#include "fk_internal.h"
+
+namespace fkd {
+
+__device__ __forceinline__ void unravel(const FkGrid& g, long long j, int idx[3]) {
+  idx[0] = idx[1] = idx[2] = 0;
+  unsigned r = (unsigned)j;                       // J * 32 < 2^31 is checked by fk_create
+  for (int k = g.d - 1; k > 0; --k) {
+    const unsigned n = (unsigned)g.n[k];
+    const unsigned q = r / n;
+    idx[k] = (int)(r - q * n);
+    r = q;
+  }
+  idx[0] = (int)r;
+}
+
+// node on an ABSORB face?  lowest dimension decides the value (R9)
+__device__ __forceinline__ bool dirichlet(const FkGrid& g, const int idx[3], double* val) {
+  for (int k = 0; k < g.d; ++k) {
+    if (idx[k] == 0 && g.face_kind[k][0] == 0) { *val = g.face_value[k][0]; return true; }
+    if (idx[k] == g.n[k] - 1 && g.face_kind[k][1] == 0) { *val = g.face_value[k][1]; return true; }
+  }
+  return false;
+}
+
+// cell c with x[c] <= z < x[c+1], 0 <= c <= n-2 (z == x[n-1] falls in the last cell); z is
+// inside [lo, hi] here.  The index is clamped whatever z is, so a NaN coefficient can only
+// produce NaN values, never an out-of-range access.
+__device__ __forceinline__ int locate(const FkGrid& g, int k, double z) {
+  const double* __restrict__ x = g.x[k];
+  const int n = g.n[k];
+  int c;
+  if (g.uniform[k]) {
+    c = __double2int_rd((z - g.lo[k]) * g.inv_h0[k]);
+    c = max(0, min(c, n - 2));
+    while (c > 0 && z < x[c]) --c;
+    while (c < n - 2 && z >= x[c + 1]) ++c;
+  } else {
+    int lo = 0, hi = n - 1;                 // invariant: x[lo] <= z (or lo == 0), z < x[hi] (or hi == n-1)
+    while (hi - lo > 1) {
+      int mid = (lo + hi) >> 1;
+      if (z >= x[mid]) lo = mid; else hi = mid;
+    }
+    c = min(lo, n - 2);
+  }
+  return c;
+}
+
+// Eq. 21: z_q = (x + b dt) + (sigma sqrt(2 dt)) a_q, products and sums NOT fused
+__device__ __forceinline__ double push_point(double centre, double spread, double a) {
+  return __dadd_rn(centre, __dmul_rn(spread, a));
+}
+
+// Conservative node range [first, last] that the Q_k points of one node can touch along
+// dimension k: the cells of the two extreme points (the points are ascending in q because
+// sigma >= 0), each projected onto the box.  Used both by the classifier (does a step have rows
+// that leave the fused kernel's halo?) and by fk_assemble (the per-row flag), so that the two
+// always agree.
+__device__ __forceinline__ void reach(const FkGrid& g, int k, double centre, double spread,
+                                      int* first, int* last) {
+  double z0 = push_point(centre, spread, g.gh_a[k][0]);
+  double z1 = push_point(centre, spread, g.gh_a[k][g.Q[k] - 1]);
+  z0 = fmin(fmax(z0, g.lo[k]), g.hi[k]);
+  z1 = fmin(fmax(z1, g.lo[k]), g.hi[k]);
+  *first = locate(g, k, fmin(z0, z1));
+  *last = locate(g, k, fmax(z0, z1)) + 1;
+}
+
+// 1/s for a normal, finite s: MUFU seed + two Newton steps (error ~1 ulp)
+__device__ __forceinline__ double rcp_newton(double s) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
+  double e = fma(-s, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-s, r, 1.0);
+  r = fma(r, e, r);
+  return r;
+}
+
+// Eq. 15: 0 if the two divided differences differ in sign or one is 0
+// (R7), else their harmonic mean 2ab/(a+b).  p = ab > 0 implies |a+b| >= 2 sqrt(p) is a normal
+// number, so the reciprocal needs no special cases; an underflowing product gives slope 0,
+// which differs from the exact value by less than 1e-150.
+__device__ __forceinline__ double harmonic(double a, double b) {
+  const double p = a * b;
+  const double r = rcp_newton(a + b);
+  return p > 0.0 ? (p + p) * r : 0.0;
+}
+
+}  // namespace fkd
+
+#endif

@@ -1,0 +1,257 @@
+// fk_fused2d.cu -- the fused 2-D step kernel: PCHIP slopes (Eq. 15) and the
+// row contraction P(:, n:N) <- A_nu [P; dP](:, n:N) in one pass, so that P is
+// read once and written once per step (16 B per node-step update) and dP never exists in HBM.
+//
+// Work decomposition.  Lane = output-time column of a 32-column chunk (as everywhere in this
+// library), so a node is one 256-byte row and the operator row is warp-uniform.  A block owns
+// a strip of T1 nodes along dimension 1 (the fast one) and marches along dimension 0 over a
+// segment of lines.  Shared memory holds a rolling window of lines:
+//     u   LBU = 2H+3 lines of T1+2H+2 nodes      (TMA bulk copies, one line ahead)
+//     d0  LBD = 2H+1 lines of T1+2H   nodes      (computed once per node of the strip + halo)
+//     d1  same
+//     rec 2 lines of T1 compact operator records (bulk copy, one line ahead)
+// Per output line i0: [prefetch u(i0+H+2), rec(i0+1)] -> contraction of line i0 from shared
+// memory -> wait/sync -> slopes of line i0+H+1 -> sync.  Slopes are recomputed only in the
+// dimension-1 halo (2H nodes per T1) and in the H0+... lines of a segment's prologue.
+//
+// Rows whose entries leave the halo (not FK_ROW_NEAR) are skipped here; the host runs the
+// generic slopes + apply kernels on them in the same step (fk_api.cu).
+#include <cstdint>
+
+#include "fk_device.cuh"
+
+namespace {
+
+constexpr int H = FK_H;
+constexpr int LBU = 2 * H + 3;
+constexpr int LBD = 2 * H + 1;
+
+template <int T1>
+struct Tile {
+  static constexpr int W1 = T1 + 2 * H;       // nodes of a slope line
+  static constexpr int WU = W1 + 2;           // nodes of a u line
+  static constexpr int NWARPS = T1 / 2;       // two rows per warp and line
+  static constexpr size_t U_ELEMS = (size_t)LBU * WU * FK_CW;
+  static constexpr size_t D_ELEMS = (size_t)LBD * W1 * FK_CW;
+  static constexpr size_t SMEM = (U_ELEMS + 2 * D_ELEMS) * sizeof(double) +
+                                 2 * T1 * sizeof(FkRec2) + 16;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes,
+                                         uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+          "r"(smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+
+// position of grid node i1 inside a u line / a slope line of the strip starting at s1
+#define FK_UPOS(i1) ((i1) - (s1 - H - 1))
+#define FK_DPOS(i1) ((i1) - (s1 - H))
+
+template <int T1>
+__device__ __forceinline__ void slopes_line(const FkGrid& g, const double* __restrict__ su,
+                                            double* __restrict__ sd0, double* __restrict__ sd1,
+                                            int l, int s1, int warp, int lane) {
+  using T = Tile<T1>;
+  const int n0 = g.n[0], n1 = g.n[1];
+  // the three consecutive lines / nodes whose two divided differences give the slope:
+  // (i-1, i, i+1) inside, the first / last three at the ends (R6)
+  const int la = min(max(l - 1, 0), n0 - 3);
+  const double iha = g.inv_h[0][la], ihb = g.inv_h[0][la + 1];
+  const double* __restrict__ ua = su + (size_t)(((unsigned)la % LBU) * T::WU) * FK_CW + lane;
+  const double* __restrict__ ub = su + (size_t)(((unsigned)(la + 1) % LBU) * T::WU) * FK_CW + lane;
+  const double* __restrict__ uc = su + (size_t)(((unsigned)(la + 2) % LBU) * T::WU) * FK_CW + lane;
+  const double* __restrict__ ul = su + (size_t)(((unsigned)l % LBU) * T::WU) * FK_CW + lane;
+  double* __restrict__ o0 = sd0 + (size_t)(((unsigned)l % LBD) * T::W1) * FK_CW + lane;
+  double* __restrict__ o1 = sd1 + (size_t)(((unsigned)l % LBD) * T::W1) * FK_CW + lane;
+  const int lo = max(0, s1 - H), hi = min(n1, s1 + T1 + H);
+  for (int i1 = lo + warp; i1 < hi; i1 += T::NWARPS) {
+    const int pu = FK_UPOS(i1) * FK_CW;
+    const double va = ua[pu], vb = ub[pu], vc = uc[pu];
+    const int ia = min(max(i1 - 1, 0), n1 - 3);
+    const double* __restrict__ q = ul + FK_UPOS(ia) * FK_CW;
+    const double wa = q[0], wb = q[FK_CW], wc = q[2 * FK_CW];
+    const double jha = g.inv_h[1][ia], jhb = g.inv_h[1][ia + 1];
+    const int pd = FK_DPOS(i1) * FK_CW;
+    o0[pd] = fkd::harmonic((vb - va) * iha, (vc - vb) * ihb);
+    o1[pd] = fkd::harmonic((wb - wa) * jha, (wc - wb) * jhb);
+  }
+}
+
+// bytes and copies of one u line (nodes of the strip + halo + 1 that exist in the grid)
+template <int T1>
+__device__ __forceinline__ uint32_t u_line_bytes(const FkGrid& g, int s1) {
+  const int a = max(0, s1 - H - 1), b = min(g.n[1], s1 + T1 + H + 1);
+  return (uint32_t)(b - a) * FK_CW * sizeof(double);
+}
+template <int T1>
+__device__ __forceinline__ void u_line_copy(const FkGrid& g, const double* __restrict__ Pc,
+                                            double* su, int l, int s1, uint64_t* bar) {
+  using T = Tile<T1>;
+  const int a = max(0, s1 - H - 1);
+  bulk_g2s(su + ((size_t)((unsigned)l % LBU) * T::WU + FK_UPOS(a)) * FK_CW,
+           Pc + ((size_t)l * g.n[1] + a) * FK_CW, u_line_bytes<T1>(g, s1), bar);
+}
+
+template <int T1>
+__global__ void __launch_bounds__(Tile<T1>::NWARPS * 32)
+fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ Pold,
+           double* __restrict__ Pnew, int chunk0, int n, int N, int nstrips, int seg_len) {
+  using T = Tile<T1>;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* su = reinterpret_cast<double*>(smem_raw);
+  double* sd0 = su + T::U_ELEMS;
+  double* sd1 = sd0 + T::D_ELEMS;
+  FkRec2* srec = reinterpret_cast<FkRec2*>(sd1 + T::D_ELEMS);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(srec + 2 * T1);
+
+  const int lane = threadIdx.x, warp = threadIdx.y;
+  const bool leader = lane == 0 && warp == 0;
+  const int n0 = g.n[0], n1 = g.n[1];
+  const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
+  const int s1 = strip * T1;
+  const int L0 = seg * seg_len, L1 = min(n0, L0 + seg_len);
+  const int chunk = chunk0 + blockIdx.y;
+  const size_t chunk_elems = (size_t)g.J * FK_CW;
+  const double* __restrict__ Pc = Pold + (size_t)chunk * chunk_elems;
+  double* __restrict__ Pn = Pnew + (size_t)chunk * chunk_elems;
+  const int rows = min(T1, n1 - s1);                      // rows of this strip
+  const uint32_t rec_bytes = (uint32_t)rows * sizeof(FkRec2);
+  const uint32_t ubytes = u_line_bytes<T1>(g, s1);
+  const int m = chunk * FK_CW + lane;
+  const bool active = m >= n && m <= N;
+
+  if (leader) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  uint32_t parity = 0;
+
+  // prologue: u lines L0-H-1 .. L0+H+1 and the records of line L0
+  {
+    const int a = max(0, L0 - H - 1), b = min(n0, L0 + H + 2);
+    if (leader) {
+      mbar_expect_tx(bar, (uint32_t)(b - a) * ubytes + rec_bytes);
+      for (int l = a; l < b; ++l) u_line_copy<T1>(g, Pc, su, l, s1, bar);
+      bulk_g2s(srec + (L0 & 1) * T1, rec + (size_t)L0 * n1 + s1, rec_bytes, bar);
+    }
+    mbar_wait(bar, parity);
+    parity ^= 1;
+    const int c = max(0, L0 - H), d = min(n0, L0 + H + 1);
+    for (int l = c; l < d; ++l) slopes_line<T1>(g, su, sd0, sd1, l, s1, warp, lane);
+    __syncthreads();
+  }
+
+  for (int i0 = L0; i0 < L1; ++i0) {
+    const int lu = i0 + H + 2;                             // u line to fetch now
+    const bool want_rec = i0 + 1 < L1, want_u = want_rec && lu < n0;
+    if (leader && (want_u || want_rec)) {
+      mbar_expect_tx(bar, (want_u ? ubytes : 0u) + (want_rec ? rec_bytes : 0u));
+      if (want_u) u_line_copy<T1>(g, Pc, su, lu, s1, bar);
+      if (want_rec)
+        bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, bar);
+    }
+
+    // ---- contraction of line i0: Eq. 13 with the quadrature weights folded in
+    const FkRec2* __restrict__ line_rec = srec + (i0 & 1) * T1;
+    for (int r = warp; r < rows; r += T::NWARPS) {
+      const FkRec2* __restrict__ rc = line_rec + r;
+      const int flags = rc->flags;
+      if (!(flags & (FK_ROW_NEAR | FK_ROW_DIRICHLET))) continue;   // far row: generic kernels
+      const int cnt0 = rc->cnt[0], cnt1 = rc->cnt[1];
+      const int p1 = rc->s[1];
+      double acc = rc->c;
+      for (int e0 = 0; e0 < cnt0; ++e0) {
+        const int line = rc->s[0] + e0;
+        const double* __restrict__ up = su + ((size_t)((unsigned)line % LBU) * T::WU + FK_UPOS(p1)) * FK_CW + lane;
+        const size_t dofs = ((size_t)((unsigned)line % LBD) * T::W1 + FK_DPOS(p1)) * FK_CW + lane;
+        const double* __restrict__ d0p = sd0 + dofs;
+        const double* __restrict__ d1p = sd1 + dofs;
+        double A = 0.0, A2 = 0.0, B0 = 0.0;
+#pragma unroll
+        for (int e1 = 0; e1 < FK_NW; ++e1) {
+          if (e1 < cnt1) {
+            const double2 w1 = rc->w[1][e1];
+            A = fma(w1.x, up[e1 * FK_CW], A);
+            A2 = fma(w1.y, d1p[e1 * FK_CW], A2);
+            B0 = fma(w1.x, d0p[e1 * FK_CW], B0);
+          }
+        }
+        const double2 w0 = rc->w[0][e0];
+        acc = fma(w0.x, A + A2, acc);
+        acc = fma(w0.y, B0, acc);
+      }
+      if (active) Pn[((size_t)i0 * n1 + s1 + r) * FK_CW + lane] = acc;
+    }
+
+    if (want_u || want_rec) {
+      mbar_wait(bar, parity);
+      parity ^= 1;
+    }
+    __syncthreads();                                       // line i0 is done with its buffers
+    const int ld = i0 + H + 1;                             // slopes of the next line to enter
+    if (ld < n0 && i0 + 1 < L1) {
+      slopes_line<T1>(g, su, sd0, sd1, ld, s1, warp, lane);
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace
+
+cudaError_t fk_fused2d_setup(void) {
+  cudaError_t e = cudaFuncSetAttribute(fk_fused2d<16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)Tile<16>::SMEM);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(fk_fused2d<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)Tile<32>::SMEM);
+}
+
+cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold, double* Pnew,
+                              int chunk0, int chunk1, int n, int N, int sm_count,
+                              cudaStream_t s) {
+  constexpr int T1 = 16;
+  const int n0 = g.n[0], n1 = g.n[1];
+  const int nstrips = (n1 + T1 - 1) / T1;
+  const int nchunks = chunk1 - chunk0;
+  // enough blocks for about four waves of two blocks per SM, segments of at least 16 lines
+  const long long want = 4LL * 2 * sm_count;
+  long long nseg = (want + (long long)nstrips * nchunks - 1) / ((long long)nstrips * nchunks);
+  const int max_seg = n0 / 16 > 1 ? n0 / 16 : 1;
+  if (nseg > max_seg) nseg = max_seg;
+  if (nseg < 1) nseg = 1;
+  const int seg_len = (int)((n0 + nseg - 1) / nseg);
+  nseg = (n0 + seg_len - 1) / seg_len;
+  dim3 block(FK_CW, Tile<T1>::NWARPS), grid((unsigned)(nstrips * nseg), (unsigned)nchunks);
+  fk_fused2d<T1><<<grid, block, Tile<T1>::SMEM, s>>>(g, op.rec, Pold, Pnew, chunk0, n, N,
+                                                      nstrips, seg_len);
+  return cudaGetLastError();
+}

@@ -40,22 +40,54 @@ struct FkGrid {
   double gh_w[3][FK_QMAX];
 };
 
+// Row flags kept in cnt[j][3]
+#define FK_ROW_DIRICHLET 1   // node on an ABSORB face: the row is the constant c_j = g
+#define FK_ROW_NEAR 2        // every entry lies within FK_H nodes of the row's node in each
+                             // dimension: the row has a compact record for the fused kernel
+
+#define FK_H 2               // halo of the fused 2-D kernel (nodes per side and dimension)
+#define FK_NW (2 * FK_H + 1) // entries per dimension of a compact record
+
+// Compact record of a near row (2-D): per dimension a run of cnt_k <= FK_NW CONSECUTIVE nodes
+// starting at node s[k] with their (alpha, beta); nodes of the run no point touches have
+// zero weights.  192 bytes, 16-byte aligned, so a line of records is one bulk copy.
+struct FkRec2 {
+  double c;               // absorbed constant (= g on Dirichlet nodes)
+  int s[2];               // first node of the run per dimension
+  int cnt[2];             // run length per dimension (0, 0 on Dirichlet rows)
+  int flags;              // FK_ROW_*
+  int pad;
+  double2 w[2][FK_NW];
+};
+
 struct FkOperator {       // device pointers of one assembled A_nu
   double2* w;             // [J][RS] (alpha, beta)
   int* off;               // [J][RS] element offset i_k*stride_k*FK_CW inside a chunk
-  int* cnt;               // [J][4]  entries used per dimension
+  int* cnt;               // [J][4]  entries used per dimension; [3] = FK_ROW_* flags
   double* c;              // [J]     absorbed constant (= g on Dirichlet nodes)
+  FkRec2* rec;            // [J]     compact records (2-D grids only, else NULL)
 };
 
 // launchers (fk_kernels.cu); all asynchronous on `s`, return the launch's cudaError_t
 cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStream_t s);
 cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
                                FkOperator op, cudaStream_t s);
+// far_rows[slot] = number of rows of the step held in that coefficient slot that are not
+// FK_ROW_NEAR (2-D only), for the `count` steps step0.. whose slices sit at
+// coef + (step % slots) * 2*d*J (b then sigma); far_rows entries must be zeroed before
+cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, int step0,
+                               int count, int* far_rows, cudaStream_t s);
+// fused 2-D kernel: slopes + apply for the FK_ROW_NEAR and Dirichlet rows of every active
+// column; P never leaves the chip between the two (fk_fused2d.cu)
+cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold, double* Pnew,
+                              int chunk0, int chunk1, int n, int N, int sm_count,
+                              cudaStream_t s);
+cudaError_t fk_fused2d_setup(void);
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
                              int chunk0, int chunk1, cudaStream_t s);
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
                             double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
-                            cudaStream_t s);
+                            int far_only, cudaStream_t s);
 cudaError_t fk_launch_gather_columns(const FkGrid& g, const double* P, int m0, int m1,
                                      double* out, cudaStream_t s);
 

@@ -12,27 +12,14 @@
 // warp = one node.  Every P / dP access of a warp is one aligned 256-byte row whatever the
 // shape of the stencil (scattered 1-D rows with Q = 16, clamped rows that reach across the
 // whole box, ...), and the operator row is warp-uniform, so it is fetched by broadcast loads.
-#include "fk_internal.h"
+#include "fk_device.cuh"
 
 namespace {
 
-__device__ __forceinline__ void unravel(const FkGrid& g, long long j, int idx[3]) {
-  idx[0] = idx[1] = idx[2] = 0;
-  for (int k = g.d - 1; k >= 0; --k) {
-    long long q = j / g.n[k];
-    idx[k] = (int)(j - q * g.n[k]);
-    j = q;
-  }
-}
-
-// node on an ABSORB face?  lowest dimension decides the value (R9)
-__device__ __forceinline__ bool dirichlet(const FkGrid& g, const int idx[3], double* val) {
-  for (int k = 0; k < g.d; ++k) {
-    if (idx[k] == 0 && g.face_kind[k][0] == 0) { *val = g.face_value[k][0]; return true; }
-    if (idx[k] == g.n[k] - 1 && g.face_kind[k][1] == 0) { *val = g.face_value[k][1]; return true; }
-  }
-  return false;
-}
+using fkd::unravel;
+using fkd::dirichlet;
+using fkd::locate;
+using fkd::harmonic;
 
 // ------------------------------------------------------------------------------------------
 // chi into every lane of every chunk (also the padding columns beyond N)
@@ -49,31 +36,6 @@ __global__ void fk_fill_chi(FkGrid g, double* __restrict__ P, int n_chunks) {
 }
 
 // ------------------------------------------------------------------------------------------
-// cell c with x[c] <= z < x[c+1], 0 <= c <= n-2 (z == x[n-1] falls in the last cell); z is
-// inside [lo, hi] here.  The index is clamped whatever z is, so a NaN coefficient can only
-// produce NaN values, never an out-of-range access.
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ int locate(const FkGrid& g, int k, double z) {
-  const double* __restrict__ x = g.x[k];
-  const int n = g.n[k];
-  int c;
-  if (g.uniform[k]) {
-    c = __double2int_rd((z - g.lo[k]) * g.inv_h0[k]);
-    c = max(0, min(c, n - 2));
-    while (c > 0 && z < x[c]) --c;
-    while (c < n - 2 && z >= x[c + 1]) ++c;
-  } else {
-    int lo = 0, hi = n - 1;                 // invariant: x[lo] <= z (or lo == 0), z < x[hi] (or hi == n-1)
-    while (hi - lo > 1) {
-      int mid = (lo + hi) >> 1;
-      if (z >= x[mid]) lo = mid; else hi = mid;
-    }
-    c = min(lo, n - 2);
-  }
-  return c;
-}
-
-// ------------------------------------------------------------------------------------------
 // fk_assemble: one thread per node.  For each dimension k the Q_k points
 //   z_q = (x + b dt) + (sigma sqrt(2 dt)) a_q          (Eq. 21; products and sums NOT fused,
 //                                                       so cells agree with any fp64 reading)
@@ -82,6 +44,9 @@ __device__ __forceinline__ int locate(const FkGrid& g, int k, double z) {
 // window that is flushed to the row as it moves.  Points outside an ABSORB face add
 // w_q * g to e_k; CLAMP faces project the point.  With m_k the inside mass of dimension k,
 //   c_j = sum_k (prod_{l<k} m_l) e_k                   (lowest outside dimension decides, R9).
+// In 2-D the row is also written as a compact record (FkRec2) when fkd::reach says that all
+// its entries stay within FK_H nodes of the row's node: the run of consecutive nodes
+// [first, last] of each dimension, zero-filled where no point lands.
 // ------------------------------------------------------------------------------------------
 __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
                             const double* __restrict__ sigma, FkOperator op) {
@@ -90,30 +55,57 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
   int idx[3];
   unravel(g, j, idx);
   int* cnt = op.cnt + j * 4;
+  FkRec2* rec = op.rec ? op.rec + j : nullptr;
   double gval;
   if (dirichlet(g, idx, &gval)) {
     cnt[0] = cnt[1] = cnt[2] = 0;
-    cnt[3] = 1;
+    cnt[3] = FK_ROW_DIRICHLET;
     op.c[j] = gval;
+    if (rec) {
+      rec->c = gval;
+      rec->s[0] = rec->s[1] = 0;
+      rec->cnt[0] = rec->cnt[1] = 0;
+      rec->flags = FK_ROW_DIRICHLET;
+    }
     return;
   }
   double2* __restrict__ roww = op.w + (size_t)j * g.RS;
   int* __restrict__ rowo = op.off + (size_t)j * g.RS;
   double cj = 0.0, mass = 1.0;
+  bool near = rec != nullptr;
   for (int k = 0; k < g.d; ++k) {
     const double xk = g.x[k][idx[k]];
     const double centre = __dadd_rn(xk, __dmul_rn(b[(size_t)k * g.J + j], g.dt));
     const double spread = __dmul_rn(sigma[(size_t)k * g.J + j], g.sq);
     const double lo = g.lo[k], hi = g.hi[k];
     const long long unit = g.stride[k] * FK_CW;
+    int first = 0, last = -1;
+    bool rec_k = false;
+    if (rec) {
+      fkd::reach(g, k, centre, spread, &first, &last);
+      rec_k = first >= idx[k] - FK_H && last <= idx[k] + FK_H;
+      near = near && rec_k;
+      if (rec_k) {
+        rec->s[k] = first;
+        rec->cnt[k] = last - first + 1;
+        for (int e = 0; e < FK_NW; ++e) rec->w[k][e] = make_double2(0.0, 0.0);
+      }
+    }
     double ek = 0.0, mk = 0.0;
     int count = 0;
     int cprev = -2;
     double aL = 0.0, bL = 0.0, aR = 0.0, bR = 0.0;
     double2* wk = roww + g.qoff[k];
     int* ok = rowo + g.qoff[k];
+#define FK_EMIT(node, A, B)                                               \
+    do {                                                                  \
+      wk[count] = make_double2((A), (B));                                 \
+      ok[count] = (int)((node) * unit);                                   \
+      ++count;                                                            \
+      if (rec_k) rec->w[k][(node) - first] = make_double2((A), (B));      \
+    } while (0)
     for (int q = 0; q < g.Q[k]; ++q) {
-      double z = __dadd_rn(centre, __dmul_rn(spread, g.gh_a[k][q]));
+      double z = fkd::push_point(centre, spread, g.gh_a[k][q]);
       const double w = g.gh_w[k][q];
       if (z < lo) {
         if (g.face_kind[k][0] == 1) z = lo; else { ek += w * g.face_value[k][0]; continue; }
@@ -134,39 +126,64 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
       if (c == cprev) {
         aL += vL; bL += sL; aR += vR; bR += sR;
       } else if (c == cprev + 1) {
-        wk[count] = make_double2(aL, bL); ok[count] = (int)(cprev * unit); ++count;
+        FK_EMIT(cprev, aL, bL);
         aL = aR + vL; bL = bR + sL; aR = vR; bR = sR;
         cprev = c;
       } else {
         if (cprev >= 0) {
-          wk[count] = make_double2(aL, bL); ok[count] = (int)(cprev * unit); ++count;
-          wk[count] = make_double2(aR, bR); ok[count] = (int)((cprev + 1) * unit); ++count;
+          FK_EMIT(cprev, aL, bL);
+          FK_EMIT(cprev + 1, aR, bR);
         }
         aL = vL; bL = sL; aR = vR; bR = sR;
         cprev = c;
       }
     }
     if (cprev >= 0) {
-      wk[count] = make_double2(aL, bL); ok[count] = (int)(cprev * unit); ++count;
-      wk[count] = make_double2(aR, bR); ok[count] = (int)((cprev + 1) * unit); ++count;
+      FK_EMIT(cprev, aL, bL);
+      FK_EMIT(cprev + 1, aR, bR);
     }
+#undef FK_EMIT
     cnt[k] = count;
     cj += mass * ek;
     mass *= mk;
   }
   for (int k = g.d; k < 3; ++k) cnt[k] = 0;
-  cnt[3] = 0;
+  cnt[3] = near ? FK_ROW_NEAR : 0;
   op.c[j] = cj;
+  if (rec) {
+    rec->c = cj;
+    rec->flags = near ? FK_ROW_NEAR : 0;
+  }
 }
 
-
 // ------------------------------------------------------------------------------------------
-// Eq. 15: 0 if the two divided differences differ in sign or one is 0 (R7), else their
-// harmonic mean 2ab/(a+b) (same-sign operands: the sum does not cancel).
+// fk_classify (2-D): how many rows of each loaded step are not FK_ROW_NEAR, by the same
+// fkd::reach test fk_assemble applies.  grid = (node blocks, steps); one atomic per warp.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ double harmonic(double a, double b) {
-  const bool same = (a > 0.0 && b > 0.0) || (a < 0.0 && b < 0.0);
-  return same ? (2.0 * a * b) / (a + b) : 0.0;
+__global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots, int step0,
+                            int* __restrict__ far_rows) {
+  const int slot = (step0 + (int)blockIdx.y) % slots;
+  const size_t slice = (size_t)g.d * g.J;
+  const double* __restrict__ b = coef + (size_t)slot * 2 * slice;
+  const double* __restrict__ sigma = b + slice;
+  long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool far = false;
+  if (j < g.J) {
+    int idx[3];
+    unravel(g, j, idx);
+    double gval;
+    if (!dirichlet(g, idx, &gval)) {
+      for (int k = 0; k < g.d; ++k) {
+        const double centre = __dadd_rn(g.x[k][idx[k]], __dmul_rn(b[(size_t)k * g.J + j], g.dt));
+        const double spread = __dmul_rn(sigma[(size_t)k * g.J + j], g.sq);
+        int first, last;
+        fkd::reach(g, k, centre, spread, &first, &last);
+        far = far || !(first >= idx[k] - FK_H && last <= idx[k] + FK_H);
+      }
+    }
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, far);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(far_rows + slot, __popc(m));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -218,7 +235,7 @@ template <int D>
 __global__ void __launch_bounds__(256)
 fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
          const double* __restrict__ dP, double* __restrict__ Pnew, int n_chunks, int chunk0,
-         int n, int N) {
+         int n, int N, int far_only) {
   long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
   if (j >= g.J) return;
   const int c = chunk0 + blockIdx.y;
@@ -231,6 +248,7 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   const double2* __restrict__ w = op.w + (size_t)j * g.RS;
   const int* __restrict__ off = op.off + (size_t)j * g.RS;
   const int4 cnt = *reinterpret_cast<const int4*>(op.cnt + j * 4);
+  if (far_only && (cnt.w & (FK_ROW_NEAR | FK_ROW_DIRICHLET))) return;   // done by fk_fused2d
   double acc = op.c[j];
   if (D == 1) {
     double a0 = 0.0, a1 = 0.0;
@@ -332,6 +350,13 @@ cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* s
   return cudaGetLastError();
 }
 
+cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, int step0,
+                               int count, int* far_rows, cudaStream_t s) {
+  dim3 grid(node_blocks(g, 128), (unsigned)count);
+  fk_classify<<<grid, 128, 0, s>>>(g, coef, slots, step0, far_rows);
+  return cudaGetLastError();
+}
+
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
                              int chunk0, int chunk1, cudaStream_t s) {
   dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(chunk1 - chunk0));
@@ -341,14 +366,14 @@ cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n
 
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
                             double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
-                            cudaStream_t s) {
+                            int far_only, cudaStream_t s) {
   dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(chunk1 - chunk0));
   if (g.d == 1)
-    fk_apply<1><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N);
+    fk_apply<1><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only);
   else if (g.d == 2)
-    fk_apply<2><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N);
+    fk_apply<2><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only);
   else
-    fk_apply<3><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N);
+    fk_apply<3><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only);
   return cudaGetLastError();
 }
 
