@@ -25,12 +25,13 @@ namespace {
 constexpr int H = FK_H;
 constexpr int LBU = 2 * H + 3;
 constexpr int LBD = 2 * H + 1;
+constexpr int RB = 4;                         // rows per warp: adjacent nodes along dimension 1
 
 template <int T1>
 struct Tile {
   static constexpr int W1 = T1 + 2 * H;       // nodes of a slope line
   static constexpr int WU = W1 + 2;           // nodes of a u line
-  static constexpr int NWARPS = T1 / 2;       // two rows per warp and line
+  static constexpr int NWARPS = T1 / RB;      // one block of RB rows per warp and line
   static constexpr size_t U_ELEMS = (size_t)LBU * WU * FK_CW;
   static constexpr size_t D_ELEMS = (size_t)LBD * W1 * FK_CW;
   static constexpr size_t SMEM = (U_ELEMS + 2 * D_ELEMS) * sizeof(double) +
@@ -75,33 +76,60 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 #define FK_UPOS(i1) ((i1) - (s1 - H - 1))
 #define FK_DPOS(i1) ((i1) - (s1 - H))
 
+// Slopes of line l (Eq. 15 along both dimensions) for the strip's slope window.  Each warp
+// owns NPW = ceil(W1 / NWARPS) consecutive nodes and sweeps them with everything in registers: the
+// NPW + 4 values of line l around them give the dimension-1 differences once each, and the
+// dimension-0 differences need two more loads per node.  Fully unrolled, so the 2 * NPW
+// harmonic means (each a chain of ~10 dependent fp64 operations) overlap.
 template <int T1>
 __device__ __forceinline__ void slopes_line(const FkGrid& g, const double* __restrict__ su,
                                             double* __restrict__ sd0, double* __restrict__ sd1,
                                             int l, int s1, int warp, int lane) {
   using T = Tile<T1>;
+  constexpr int NPW = (T::W1 + T::NWARPS - 1) / T::NWARPS;
   const int n0 = g.n[0], n1 = g.n[1];
   // the three consecutive lines / nodes whose two divided differences give the slope:
   // (i-1, i, i+1) inside, the first / last three at the ends (R6)
   const int la = min(max(l - 1, 0), n0 - 3);
   const double iha = g.inv_h[0][la], ihb = g.inv_h[0][la + 1];
-  const double* __restrict__ ua = su + (size_t)(((unsigned)la % LBU) * T::WU) * FK_CW + lane;
-  const double* __restrict__ ub = su + (size_t)(((unsigned)(la + 1) % LBU) * T::WU) * FK_CW + lane;
-  const double* __restrict__ uc = su + (size_t)(((unsigned)(la + 2) % LBU) * T::WU) * FK_CW + lane;
-  const double* __restrict__ ul = su + (size_t)(((unsigned)l % LBU) * T::WU) * FK_CW + lane;
-  double* __restrict__ o0 = sd0 + (size_t)(((unsigned)l % LBD) * T::W1) * FK_CW + lane;
-  double* __restrict__ o1 = sd1 + (size_t)(((unsigned)l % LBD) * T::W1) * FK_CW + lane;
-  const int lo = max(0, s1 - H), hi = min(n1, s1 + T1 + H);
-  for (int i1 = lo + warp; i1 < hi; i1 += T::NWARPS) {
-    const int pu = FK_UPOS(i1) * FK_CW;
-    const double va = ua[pu], vb = ub[pu], vc = uc[pu];
-    const int ia = min(max(i1 - 1, 0), n1 - 3);
-    const double* __restrict__ q = ul + FK_UPOS(ia) * FK_CW;
-    const double wa = q[0], wb = q[FK_CW], wc = q[2 * FK_CW];
-    const double jha = g.inv_h[1][ia], jhb = g.inv_h[1][ia + 1];
-    const int pd = FK_DPOS(i1) * FK_CW;
-    o0[pd] = fkd::harmonic((vb - va) * iha, (vc - vb) * ihb);
-    o1[pd] = fkd::harmonic((wb - wa) * jha, (wc - wb) * jhb);
+  const double* __restrict__ ua = su + (((unsigned)la % LBU) * T::WU) * FK_CW + lane;
+  const double* __restrict__ ub = su + (((unsigned)(la + 1) % LBU) * T::WU) * FK_CW + lane;
+  const double* __restrict__ uc = su + (((unsigned)(la + 2) % LBU) * T::WU) * FK_CW + lane;
+  const double* __restrict__ ul = su + (((unsigned)l % LBU) * T::WU) * FK_CW + lane;
+  double* __restrict__ o0 = sd0 + (((unsigned)l % LBD) * T::W1) * FK_CW + lane;
+  double* __restrict__ o1 = sd1 + (((unsigned)l % LBD) * T::W1) * FK_CW + lane;
+  const int p0 = warp * NPW;                       // first slope-window position of this warp
+  const int i_first = s1 - H + p0;                 // its grid node
+  // values of line l at nodes i_first-2 .. i_first+NPW+1 (u-window positions p0-1 ..), each
+  // clamped into the part of the window that exists; clamped duplicates are never selected
+  const int wlo = max(0, s1 - H - 1), whi = min(n1, s1 + T1 + H + 1) - 1;
+  double v[NPW + 4];
+#pragma unroll
+  for (int k = 0; k < NPW + 4; ++k) {
+    const int i1 = min(max(i_first - 2 + k, wlo), whi);
+    v[k] = ul[FK_UPOS(i1) * FK_CW];
+  }
+  double dl[NPW + 3];                               // dl[k] = difference between v[k+1], v[k]
+#pragma unroll
+  for (int k = 0; k < NPW + 3; ++k) {
+    const int i1 = min(max(i_first - 2 + k, 0), n1 - 2);
+    dl[k] = (v[k + 1] - v[k]) * g.inv_h[1][i1];
+  }
+#pragma unroll
+  for (int k = 0; k < NPW; ++k) {
+    const int i1 = i_first + k;
+    if (i1 >= 0 && i1 < n1 && p0 + k < T::W1) {
+      // node i1 is v[k+2]; inside: (dl[k+1], dl[k+2]); first node: (dl[k+2], dl[k+3]); last
+      // node: (dl[k], dl[k+1])
+      const double a = i1 == 0 ? dl[k + 2] : (i1 == n1 - 1 ? dl[k] : dl[k + 1]);
+      const double b = i1 == 0 ? dl[k + 3] : (i1 == n1 - 1 ? dl[k + 1] : dl[k + 2]);
+      const int pu = FK_UPOS(i1) * FK_CW;
+      const double va = ua[pu], vc = uc[pu];
+      const double vb = (la + 1 == l) ? v[k + 2] : ub[pu];
+      const int pd = (p0 + k) * FK_CW;
+      o0[pd] = fkd::harmonic((vb - va) * iha, (vc - vb) * ihb);
+      o1[pd] = fkd::harmonic(a, b);
+    }
   }
 }
 
@@ -170,6 +198,11 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
     __syncthreads();
   }
 
+  // union node q of a warp's RB rows is grid node s1 + RB*warp - H + q; element offsets of
+  // q = 0 inside a u / slope line, made opaque so that they stay in registers
+  int ucol = (RB * warp + 1) * FK_CW + lane, dcol = (RB * warp) * FK_CW + lane;
+  asm volatile("" : "+r"(ucol), "+r"(dcol));
+
   for (int i0 = L0; i0 < L1; ++i0) {
     const int lu = i0 + H + 2;                             // u line to fetch now
     const bool want_rec = i0 + 1 < L1, want_u = want_rec && lu < n0;
@@ -180,36 +213,72 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
         bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, bar);
     }
 
-    // ---- contraction of line i0: Eq. 13 with the quadrature weights folded in
-    const FkRec2* __restrict__ line_rec = srec + (i0 & 1) * T1;
-    for (int r = warp; r < rows; r += T::NWARPS) {
-      const FkRec2* __restrict__ rc = line_rec + r;
-      const int flags = rc->flags;
-      if (!(flags & (FK_ROW_NEAR | FK_ROW_DIRICHLET))) continue;   // far row: generic kernels
-      const int cnt0 = rc->cnt[0], cnt1 = rc->cnt[1];
-      const int p1 = rc->s[1];
-      double acc = rc->c;
-      for (int e0 = 0; e0 < cnt0; ++e0) {
-        const int line = rc->s[0] + e0;
-        const double* __restrict__ up = su + ((size_t)((unsigned)line % LBU) * T::WU + FK_UPOS(p1)) * FK_CW + lane;
-        const size_t dofs = ((size_t)((unsigned)line % LBD) * T::W1 + FK_DPOS(p1)) * FK_CW + lane;
-        const double* __restrict__ d0p = sd0 + dofs;
-        const double* __restrict__ d1p = sd1 + dofs;
-        double A = 0.0, A2 = 0.0, B0 = 0.0;
+    // ---- contraction of line i0 (Eq. 13 with the quadrature weights folded in).  A warp
+    // takes RB adjacent rows; their (2H+1)-node windows along dimension 1 overlap, so every
+    // u / d0 / d1 value of the union window is loaded once and used by up to 2H+1 rows.  All
+    // register indices are static: slot t of row r is union node q = r + t.
+    {
+      const FkRec2* __restrict__ rc = srec + (i0 & 1) * T1 + warp * RB;
+      double2 w1[RB][FK_NW];
+      double acc[RB];
+      unsigned m1[RB];
+      unsigned lines = 0, nodes = 0;
+      bool store[RB];
 #pragma unroll
-        for (int e1 = 0; e1 < FK_NW; ++e1) {
-          if (e1 < cnt1) {
-            const double2 w1 = rc->w[1][e1];
-            A = fma(w1.x, up[e1 * FK_CW], A);
-            A2 = fma(w1.y, d1p[e1 * FK_CW], A2);
-            B0 = fma(w1.x, d0p[e1 * FK_CW], B0);
+      for (int r = 0; r < RB; ++r) {
+        const bool valid = warp * RB + r < rows;
+        const int flags = valid ? rc[r].flags : 0;
+        const bool mine = (flags & (FK_ROW_NEAR | FK_ROW_DIRICHLET)) != 0;
+        store[r] = mine && active;
+        m1[r] = mine ? (unsigned)rc[r].mask[1] : 0u;
+        lines |= mine ? (unsigned)rc[r].mask[0] : 0u;
+        nodes |= m1[r] << r;
+        acc[r] = valid ? rc[r].c : 0.0;
+#pragma unroll
+        for (int t = 0; t < FK_NW; ++t) w1[r][t] = rc[r].w[1][t];
+      }
+      // the masks are the same in every lane; the reductions tell the compiler so (uniform
+      // registers, plain branches instead of divergence bookkeeping)
+      lines = __reduce_or_sync(0xffffffffu, lines);
+      nodes = __reduce_or_sync(0xffffffffu, nodes);
+      int uslot = (unsigned)(i0 + LBU - H) % LBU, dslot = (unsigned)(i0 + LBD - H) % LBD;
+      for (int t0 = 0; t0 < FK_NW; ++t0) {
+        if ((lines >> t0) & 1u) {
+          const double* __restrict__ up = su + (uslot * (T::WU * FK_CW) + ucol);
+          const double* __restrict__ d0p = sd0 + (dslot * (T::W1 * FK_CW) + dcol);
+          const double* __restrict__ d1p = d0p + T::D_ELEMS;
+          double A[RB], A2[RB], B0[RB];
+#pragma unroll
+          for (int r = 0; r < RB; ++r) A[r] = A2[r] = B0[r] = 0.0;
+#pragma unroll
+          for (int q = 0; q < RB + FK_NW - 1; ++q) {
+            // no per-node skipping: straight-line code lets the loads and the 3*RB
+            // accumulation chains of a line overlap; unused slots hold zero weights
+            const double U = up[q * FK_CW], D0 = d0p[q * FK_CW], D1 = d1p[q * FK_CW];
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+              const int t = q - r;
+              if (t >= 0 && t < FK_NW) {
+                A[r] = fma(w1[r][t].x, U, A[r]);
+                A2[r] = fma(w1[r][t].y, D1, A2[r]);
+                B0[r] = fma(w1[r][t].x, D0, B0[r]);
+              }
+            }
+          }
+#pragma unroll
+          for (int r = 0; r < RB; ++r) {
+            const double2 w0 = rc[r].w[0][t0];           // zero if row r does not use the line
+            acc[r] = fma(w0.x, A[r] + A2[r], acc[r]);
+            acc[r] = fma(w0.y, B0[r], acc[r]);
           }
         }
-        const double2 w0 = rc->w[0][e0];
-        acc = fma(w0.x, A + A2, acc);
-        acc = fma(w0.y, B0, acc);
+        uslot = uslot + 1 == LBU ? 0 : uslot + 1;
+        dslot = dslot + 1 == LBD ? 0 : dslot + 1;
       }
-      if (active) Pn[((size_t)i0 * n1 + s1 + r) * FK_CW + lane] = acc;
+      double* __restrict__ out = Pn + ((size_t)i0 * n1 + s1 + warp * RB) * FK_CW + lane;
+#pragma unroll
+      for (int r = 0; r < RB; ++r)
+        if (store[r]) out[r * FK_CW] = acc[r];
     }
 
     if (want_u || want_rec) {

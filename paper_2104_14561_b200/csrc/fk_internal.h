@@ -48,15 +48,15 @@ struct FkGrid {
 #define FK_H 2               // halo of the fused 2-D kernel (nodes per side and dimension)
 #define FK_NW (2 * FK_H + 1) // entries per dimension of a compact record
 
-// Compact record of a near row (2-D): per dimension a run of cnt_k <= FK_NW CONSECUTIVE nodes
-// starting at node s[k] with their (alpha, beta); nodes of the run no point touches have
-// zero weights.  192 bytes, 16-byte aligned, so a line of records is one bulk copy.
+// Compact record of a near row (2-D): per dimension k the FK_NW = 2*FK_H+1 weights
+// (alpha, beta) of the nodes i_k - FK_H .. i_k + FK_H around the row's own node i_k, zero where
+// no quadrature point lands (or where the node does not exist); mask[k] has bit t set where
+// slot t received an entry.  192 bytes, 16-byte aligned, so a line of records is one bulk copy.
 struct FkRec2 {
   double c;               // absorbed constant (= g on Dirichlet nodes)
-  int s[2];               // first node of the run per dimension
-  int cnt[2];             // run length per dimension (0, 0 on Dirichlet rows)
   int flags;              // FK_ROW_*
-  int pad;
+  int mask[2];            // used slots per dimension (0 on Dirichlet rows)
+  int pad[3];
   double2 w[2][FK_NW];
 };
 

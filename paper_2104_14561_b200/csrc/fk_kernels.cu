@@ -45,8 +45,8 @@ __global__ void fk_fill_chi(FkGrid g, double* __restrict__ P, int n_chunks) {
 // w_q * g to e_k; CLAMP faces project the point.  With m_k the inside mass of dimension k,
 //   c_j = sum_k (prod_{l<k} m_l) e_k                   (lowest outside dimension decides, R9).
 // In 2-D the row is also written as a compact record (FkRec2) when fkd::reach says that all
-// its entries stay within FK_H nodes of the row's node: the run of consecutive nodes
-// [first, last] of each dimension, zero-filled where no point lands.
+// its entries stay within FK_H nodes of the row's node: the weights of the 2*FK_H+1 nodes
+// around it per dimension, zero where no point lands.
 // ------------------------------------------------------------------------------------------
 __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
                             const double* __restrict__ sigma, FkOperator op) {
@@ -63,8 +63,7 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
     op.c[j] = gval;
     if (rec) {
       rec->c = gval;
-      rec->s[0] = rec->s[1] = 0;
-      rec->cnt[0] = rec->cnt[1] = 0;
+      rec->mask[0] = rec->mask[1] = 0;
       rec->flags = FK_ROW_DIRICHLET;
     }
     return;
@@ -79,17 +78,16 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
     const double spread = __dmul_rn(sigma[(size_t)k * g.J + j], g.sq);
     const double lo = g.lo[k], hi = g.hi[k];
     const long long unit = g.stride[k] * FK_CW;
-    int first = 0, last = -1;
     bool rec_k = false;
+    int rmask = 0;
+    const int rbase = idx[k] - FK_H;         // node of slot 0 of the record
     if (rec) {
+      int first, last;
       fkd::reach(g, k, centre, spread, &first, &last);
-      rec_k = first >= idx[k] - FK_H && last <= idx[k] + FK_H;
+      rec_k = first >= rbase && last <= idx[k] + FK_H;
       near = near && rec_k;
-      if (rec_k) {
-        rec->s[k] = first;
-        rec->cnt[k] = last - first + 1;
+      if (rec_k)
         for (int e = 0; e < FK_NW; ++e) rec->w[k][e] = make_double2(0.0, 0.0);
-      }
     }
     double ek = 0.0, mk = 0.0;
     int count = 0;
@@ -102,7 +100,10 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
       wk[count] = make_double2((A), (B));                                 \
       ok[count] = (int)((node) * unit);                                   \
       ++count;                                                            \
-      if (rec_k) rec->w[k][(node) - first] = make_double2((A), (B));      \
+      if (rec_k) {                                                        \
+        rec->w[k][(node) - rbase] = make_double2((A), (B));               \
+        rmask |= 1 << ((node) - rbase);                                   \
+      }                                                                   \
     } while (0)
     for (int q = 0; q < g.Q[k]; ++q) {
       double z = fkd::push_point(centre, spread, g.gh_a[k][q]);
@@ -144,6 +145,7 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
     }
 #undef FK_EMIT
     cnt[k] = count;
+    if (rec) rec->mask[k] = rmask;
     cj += mass * ek;
     mass *= mk;
   }
