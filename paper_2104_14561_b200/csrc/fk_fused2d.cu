@@ -23,19 +23,20 @@
 namespace {
 
 constexpr int H = FK_H;
-constexpr int LBU = 2 * H + 3;
-constexpr int LBD = 2 * H + 1;
+constexpr int LBU = 2 * H + 4;                // resident u lines: i0-H .. i0+H+3
+constexpr int LBD = 2 * H + 2;                // resident slope lines: i0-H .. i0+H+1
 constexpr int RB = 4;                         // rows per warp: adjacent nodes along dimension 1
 
 template <int T1>
 struct Tile {
   static constexpr int W1 = T1 + 2 * H;       // nodes of a slope line
   static constexpr int WU = W1 + 2;           // nodes of a u line
-  static constexpr int NWARPS = T1 / RB;      // one block of RB rows per warp and line
+  static constexpr int NWARPS = T1 / RB;      // warps per role: one block of RB rows each
+  static constexpr int THREADS = 2 * NWARPS * 32;   // contraction warps + slope warps
   static constexpr size_t U_ELEMS = (size_t)LBU * WU * FK_CW;
   static constexpr size_t D_ELEMS = (size_t)LBD * W1 * FK_CW;
   static constexpr size_t SMEM = (U_ELEMS + 2 * D_ELEMS) * sizeof(double) +
-                                 2 * T1 * sizeof(FkRec2) + 16;
+                                 2 * T1 * sizeof(FkRec2) + 32;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -149,7 +150,7 @@ __device__ __forceinline__ void u_line_copy(const FkGrid& g, const double* __res
 }
 
 template <int T1>
-__global__ void __launch_bounds__(Tile<T1>::NWARPS * 32)
+__global__ void __launch_bounds__(Tile<T1>::THREADS, 2)
 fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ Pold,
            double* __restrict__ Pnew, int chunk0, int n, int N, int nstrips, int seg_len) {
   using T = Tile<T1>;
@@ -158,10 +159,15 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
   double* sd0 = su + T::U_ELEMS;
   double* sd1 = sd0 + T::D_ELEMS;
   FkRec2* srec = reinterpret_cast<FkRec2*>(sd1 + T::D_ELEMS);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(srec + 2 * T1);
+  uint64_t* ubar = reinterpret_cast<uint64_t*>(srec + 2 * T1);   // u lines landed
+  uint64_t* rbar = ubar + 1;                                      // [2] operator records landed
 
-  const int lane = threadIdx.x, warp = threadIdx.y;
-  const bool leader = lane == 0 && warp == 0;
+  // roles: warps 0..NWARPS-1 contract (many registers), NWARPS..2*NWARPS-1 compute slopes and
+  // drive the TMA copies (few registers); `warp` is the index inside the role
+  const int lane = threadIdx.x;
+  const bool contractor = (int)threadIdx.y < T::NWARPS;
+  const int warp = contractor ? threadIdx.y : threadIdx.y - T::NWARPS;
+  const bool leader = lane == 0 && (int)threadIdx.y == T::NWARPS;
   const int n0 = g.n[0], n1 = g.n[1];
   const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
   const int s1 = strip * T1;
@@ -177,41 +183,82 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
   const bool active = m >= n && m <= N;
 
   if (leader) {
-    mbar_init(bar, 1);
+    mbar_init(ubar, 1);
+    mbar_init(rbar, 1);
+    mbar_init(rbar + 1, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
-  uint32_t parity = 0;
-
-  // prologue: u lines L0-H-1 .. L0+H+1 and the records of line L0
+  // Window positions that fall outside the grid are never written by the copies or the slope
+  // sweep but are read (with zero weights) by the branch-free contraction: clear the window
+  // once so that no stale NaN pattern can be multiplied by those zeros.
   {
-    const int a = max(0, L0 - H - 1), b = min(n0, L0 + H + 2);
+    double2* z = reinterpret_cast<double2*>(su);
+    const int nz = (int)((T::U_ELEMS + 2 * T::D_ELEMS) / 2);
+    for (int i = threadIdx.y * FK_CW + threadIdx.x; i < nz; i += T::THREADS)
+      z[i] = make_double2(0.0, 0.0);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // before the TMA writes
+  }
+  __syncthreads();
+
+  // prologue: u lines L0-H-1 .. L0+H+2 and the records of line L0; slopes of L0-H .. L0+H
+  {
+    const int a = max(0, L0 - H - 1), b = min(n0, L0 + H + 3);
     if (leader) {
-      mbar_expect_tx(bar, (uint32_t)(b - a) * ubytes + rec_bytes);
-      for (int l = a; l < b; ++l) u_line_copy<T1>(g, Pc, su, l, s1, bar);
-      bulk_g2s(srec + (L0 & 1) * T1, rec + (size_t)L0 * n1 + s1, rec_bytes, bar);
+      mbar_expect_tx(ubar, (uint32_t)(b - a) * ubytes);
+      for (int l = a; l < b; ++l) u_line_copy<T1>(g, Pc, su, l, s1, ubar);
+      mbar_expect_tx(rbar + (L0 & 1), rec_bytes);
+      bulk_g2s(srec + (L0 & 1) * T1, rec + (size_t)L0 * n1 + s1, rec_bytes, rbar + (L0 & 1));
     }
-    mbar_wait(bar, parity);
-    parity ^= 1;
+    mbar_wait(ubar, 0);
     const int c = max(0, L0 - H), d = min(n0, L0 + H + 1);
-    for (int l = c; l < d; ++l) slopes_line<T1>(g, su, sd0, sd1, l, s1, warp, lane);
+    for (int l = c + (contractor ? 0 : 1); l < d; l += 2)    // the two roles share the lines
+      slopes_line<T1>(g, su, sd0, sd1, l, s1, warp, lane);
     __syncthreads();
   }
 
+  if (!contractor) {
+    // ================= slope warps: per line i0, fetch u(i0+H+3) and rec(i0+1), then the
+    // slopes of line i0+H+1 (needs u up to i0+H+2, fetched one iteration earlier)
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+    uint32_t uparity = 1;
+    for (int i0 = L0; i0 < L1; ++i0) {
+      const bool more = i0 + 1 < L1;                       // a next line exists in this segment
+      const int lf = i0 + H + 3;                           // u line to fetch now
+      const int ld = i0 + H + 1;                           // slopes of the next line to enter
+      // an mbarrier phase must complete before the next one is armed: first wait for
+      // u(ld+1), fetched during iteration i0-1, then arm the fetch of u(lf)
+      if (more && i0 > L0 && ld + 1 < n0) {
+        mbar_wait(ubar, uparity);
+        uparity ^= 1;
+      }
+      if (leader) {
+        if (more && i0 + 2 < L1 && lf < n0) {              // needed by the slopes of iteration i0+1
+          mbar_expect_tx(ubar, ubytes);
+          u_line_copy<T1>(g, Pc, su, lf, s1, ubar);
+        }
+        if (more) {                                        // barrier (i0+1)&1 was consumed at i0-1
+          uint64_t* rb = rbar + ((i0 + 1) & 1);
+          mbar_expect_tx(rb, rec_bytes);
+          bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, rb);
+        }
+      }
+      if (more && ld < n0) slopes_line<T1>(g, su, sd0, sd1, ld, s1, warp, lane);
+      asm volatile("bar.sync 1, %0;" ::"n"(T::THREADS) : "memory");
+    }
+    return;
+  }
+
+  // ================= contraction warps
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
   // union node q of a warp's RB rows is grid node s1 + RB*warp - H + q; element offsets of
   // q = 0 inside a u / slope line, made opaque so that they stay in registers
   int ucol = (RB * warp + 1) * FK_CW + lane, dcol = (RB * warp) * FK_CW + lane;
   asm volatile("" : "+r"(ucol), "+r"(dcol));
+  uint32_t rparity = 0;                                    // bit b: parity to wait for on rbar[b]
 
   for (int i0 = L0; i0 < L1; ++i0) {
-    const int lu = i0 + H + 2;                             // u line to fetch now
-    const bool want_rec = i0 + 1 < L1, want_u = want_rec && lu < n0;
-    if (leader && (want_u || want_rec)) {
-      mbar_expect_tx(bar, (want_u ? ubytes : 0u) + (want_rec ? rec_bytes : 0u));
-      if (want_u) u_line_copy<T1>(g, Pc, su, lu, s1, bar);
-      if (want_rec)
-        bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, bar);
-    }
+    mbar_wait(rbar + (i0 & 1), (rparity >> (i0 & 1)) & 1u);   // records of line i0
+    rparity ^= 1u << (i0 & 1);
 
     // ---- contraction of line i0 (Eq. 13 with the quadrature weights folded in).  A warp
     // takes RB adjacent rows; their (2H+1)-node windows along dimension 1 overlap, so every
@@ -281,27 +328,15 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
         if (store[r]) out[r * FK_CW] = acc[r];
     }
 
-    if (want_u || want_rec) {
-      mbar_wait(bar, parity);
-      parity ^= 1;
-    }
-    __syncthreads();                                       // line i0 is done with its buffers
-    const int ld = i0 + H + 1;                             // slopes of the next line to enter
-    if (ld < n0 && i0 + 1 < L1) {
-      slopes_line<T1>(g, su, sd0, sd1, ld, s1, warp, lane);
-    }
-    __syncthreads();
+    asm volatile("bar.sync 1, %0;" ::"n"(T::THREADS) : "memory");
   }
 }
 
 }  // namespace
 
 cudaError_t fk_fused2d_setup(void) {
-  cudaError_t e = cudaFuncSetAttribute(fk_fused2d<16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)Tile<16>::SMEM);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(fk_fused2d<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)Tile<32>::SMEM);
+  return cudaFuncSetAttribute(fk_fused2d<16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)Tile<16>::SMEM);
 }
 
 cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold, double* Pnew,
@@ -319,7 +354,7 @@ cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold
   if (nseg < 1) nseg = 1;
   const int seg_len = (int)((n0 + nseg - 1) / nseg);
   nseg = (n0 + seg_len - 1) / seg_len;
-  dim3 block(FK_CW, Tile<T1>::NWARPS), grid((unsigned)(nstrips * nseg), (unsigned)nchunks);
+  dim3 block(FK_CW, 2 * Tile<T1>::NWARPS), grid((unsigned)(nstrips * nseg), (unsigned)nchunks);
   fk_fused2d<T1><<<grid, block, Tile<T1>::SMEM, s>>>(g, op.rec, Pold, Pnew, chunk0, n, N,
                                                       nstrips, seg_len);
   return cudaGetLastError();
