@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -36,6 +37,7 @@ struct fk_ctx {
   std::vector<int> h_far;              // host copy, valid when far_valid
   bool far_valid = false;
   int sm_count = 148;
+  bool use_tmem = false;               // fused 2-D variant: slopes in smem; FK_FUSED2D=tmem: in TMEM
   double* d_stage = nullptr;           // fk_read staging for host destinations
   size_t stage_bytes = 0;
   int n_next = 0;                      // the n the next fk_evolve must start from
@@ -270,6 +272,9 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     FK_CREATE_CUDA(cudaMalloc(&c->d_far, sizeof(int) * (size_t)slots));
     FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots, c->stream));
     FK_CREATE_CUDA(fk_fused2d_setup());
+    FK_CREATE_CUDA(fk_fused2d_tmem_setup());
+    const char* variant = std::getenv("FK_FUSED2D");
+    c->use_tmem = variant && std::strcmp(variant, "tmem") == 0;
     c->h_far.assign(slots, 0);
   }
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[0], c->n_chunks, c->stream));
@@ -399,7 +404,7 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
     const bool fused = c->g.d == 2;
     const bool generic = !fused || c->h_far[slot] > 0;   // rows the fused kernel leaves out
     if (fused)
-      FK_LAUNCH(c, FK_K_FUSED, fk_launch_fused2d(c->g, c->op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
+      FK_LAUNCH(c, FK_K_FUSED, (c->use_tmem ? fk_launch_fused2d_tmem : fk_launch_fused2d)(c->g, c->op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
     if (generic) {
       FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, c->stream));
       FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, c->stream));

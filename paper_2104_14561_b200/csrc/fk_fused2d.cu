@@ -36,42 +36,14 @@ struct Tile {
   static constexpr size_t U_ELEMS = (size_t)LBU * WU * FK_CW;
   static constexpr size_t D_ELEMS = (size_t)LBD * W1 * FK_CW;
   static constexpr size_t SMEM = (U_ELEMS + 2 * D_ELEMS) * sizeof(double) +
-                                 2 * T1 * sizeof(FkRec2) + 32;
+                                 2 * T1 * sizeof(FkRec2) + 48 + (W1 + 4) * sizeof(double);
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-               "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes,
-                                         uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
-          "r"(smem_u32(dst)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar))
-      : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra WAIT_DONE;\n"
-      "bra WAIT_LOOP;\n"
-      "WAIT_DONE:\n"
-      "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity)
-      : "memory");
-}
-
+using fkd::smem_u32;
+using fkd::mbar_init;
+using fkd::mbar_expect_tx;
+using fkd::bulk_g2s;
+using fkd::mbar_wait;
 
 // position of grid node i1 inside a u line / a slope line of the strip starting at s1
 #define FK_UPOS(i1) ((i1) - (s1 - H - 1))
@@ -85,14 +57,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 template <int T1>
 __device__ __forceinline__ void slopes_line(const FkGrid& g, const double* __restrict__ su,
                                             double* __restrict__ sd0, double* __restrict__ sd1,
-                                            int l, int s1, int warp, int lane) {
+                                            const double* __restrict__ sih, double iha,
+                                            double ihb, int l, int s1, int warp, int lane) {
   using T = Tile<T1>;
   constexpr int NPW = (T::W1 + T::NWARPS - 1) / T::NWARPS;
   const int n0 = g.n[0], n1 = g.n[1];
   // the three consecutive lines / nodes whose two divided differences give the slope:
   // (i-1, i, i+1) inside, the first / last three at the ends (R6)
   const int la = min(max(l - 1, 0), n0 - 3);
-  const double iha = g.inv_h[0][la], ihb = g.inv_h[0][la + 1];
   const double* __restrict__ ua = su + (((unsigned)la % LBU) * T::WU) * FK_CW + lane;
   const double* __restrict__ ub = su + (((unsigned)(la + 1) % LBU) * T::WU) * FK_CW + lane;
   const double* __restrict__ uc = su + (((unsigned)(la + 2) % LBU) * T::WU) * FK_CW + lane;
@@ -114,7 +86,7 @@ __device__ __forceinline__ void slopes_line(const FkGrid& g, const double* __res
 #pragma unroll
   for (int k = 0; k < NPW + 3; ++k) {
     const int i1 = min(max(i_first - 2 + k, 0), n1 - 2);
-    dl[k] = (v[k + 1] - v[k]) * g.inv_h[1][i1];
+    dl[k] = (v[k + 1] - v[k]) * sih[p0 + k];   // 1/h of the cell right of node i_first-2+k
   }
 #pragma unroll
   for (int k = 0; k < NPW; ++k) {
@@ -160,7 +132,8 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
   double* sd1 = sd0 + T::D_ELEMS;
   FkRec2* srec = reinterpret_cast<FkRec2*>(sd1 + T::D_ELEMS);
   uint64_t* ubar = reinterpret_cast<uint64_t*>(srec + 2 * T1);   // u lines landed
-  uint64_t* rbar = ubar + 1;                                      // [2] operator records landed
+  uint64_t* rbar = ubar + 2;                                      // ubar[2], rbar[2]
+  double* sih = reinterpret_cast<double*>(rbar + 2) + 1;          // 1/h table, dimension 1
 
   // roles: warps 0..NWARPS-1 contract (many registers), NWARPS..2*NWARPS-1 compute slopes and
   // drive the TMA copies (few registers); `warp` is the index inside the role
@@ -184,6 +157,7 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
 
   if (leader) {
     mbar_init(ubar, 1);
+    mbar_init(ubar + 1, 1);
     mbar_init(rbar, 1);
     mbar_init(rbar + 1, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -196,6 +170,9 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
     const int nz = (int)((T::U_ELEMS + 2 * T::D_ELEMS) / 2);
     for (int i = threadIdx.y * FK_CW + threadIdx.x; i < nz; i += T::THREADS)
       z[i] = make_double2(0.0, 0.0);
+    // sih[p] = 1/h of the cell right of grid node s1 - H - 2 + p (index clamped to the grid)
+    for (int p = threadIdx.y * FK_CW + threadIdx.x; p < T::W1 + 4; p += T::THREADS)
+      sih[p] = g.inv_h[1][min(max(s1 - H - 2 + p, 0), g.n[1] - 2)];
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // before the TMA writes
   }
   __syncthreads();
@@ -212,7 +189,10 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
     mbar_wait(ubar, 0);
     const int c = max(0, L0 - H), d = min(n0, L0 + H + 1);
     for (int l = c + (contractor ? 0 : 1); l < d; l += 2)    // the two roles share the lines
-      slopes_line<T1>(g, su, sd0, sd1, l, s1, warp, lane);
+    {
+      const int la = min(max(l - 1, 0), n0 - 3);
+      slopes_line<T1>(g, su, sd0, sd1, sih, g.inv_h[0][la], g.inv_h[0][la + 1], l, s1, warp, lane);
+    }
     __syncthreads();
   }
 
@@ -220,21 +200,27 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
     // ================= slope warps: per line i0, fetch u(i0+H+3) and rec(i0+1), then the
     // slopes of line i0+H+1 (needs u up to i0+H+2, fetched one iteration earlier)
     asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-    uint32_t uparity = 1;
+    uint32_t uparity = 1;                                  // bit b: parity to wait for on ubar[b]
     for (int i0 = L0; i0 < L1; ++i0) {
       const bool more = i0 + 1 < L1;                       // a next line exists in this segment
       const int lf = i0 + H + 3;                           // u line to fetch now
       const int ld = i0 + H + 1;                           // slopes of the next line to enter
+      // 1/h of the two line gaps around ld, issued before any wait (off the critical path)
+      const int lda = min(max(ld - 1, 0), n0 - 3);
+      const double iha = g.inv_h[0][lda], ihb = g.inv_h[0][lda + 1];
       // an mbarrier phase must complete before the next one is armed: first wait for
       // u(ld+1), fetched during iteration i0-1, then arm the fetch of u(lf)
       if (more && i0 > L0 && ld + 1 < n0) {
-        mbar_wait(ubar, uparity);
-        uparity ^= 1;
+        // two alternating barriers: a barrier is re-armed two iterations after its wait, with
+        // a block barrier in between, so no warp can miss a phase
+        const int b = (ld + 1) & 1;
+        mbar_wait(ubar + b, (uparity >> b) & 1u);
+        uparity ^= 1u << b;
       }
       if (leader) {
         if (more && i0 + 2 < L1 && lf < n0) {              // needed by the slopes of iteration i0+1
-          mbar_expect_tx(ubar, ubytes);
-          u_line_copy<T1>(g, Pc, su, lf, s1, ubar);
+          mbar_expect_tx(ubar + (lf & 1), ubytes);
+          u_line_copy<T1>(g, Pc, su, lf, s1, ubar + (lf & 1));
         }
         if (more) {                                        // barrier (i0+1)&1 was consumed at i0-1
           uint64_t* rb = rbar + ((i0 + 1) & 1);
@@ -242,7 +228,7 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
           bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, rb);
         }
       }
-      if (more && ld < n0) slopes_line<T1>(g, su, sd0, sd1, ld, s1, warp, lane);
+      if (more && ld < n0) slopes_line<T1>(g, su, sd0, sd1, sih, iha, ihb, ld, s1, warp, lane);
       asm volatile("bar.sync 1, %0;" ::"n"(T::THREADS) : "memory");
     }
     return;

@@ -83,6 +83,11 @@ cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold
                               int chunk0, int chunk1, int n, int N, int sm_count,
                               cudaStream_t s);
 cudaError_t fk_fused2d_setup(void);
+// same contract, slopes kept in tensor memory instead of shared memory (fk_fused2d_tmem.cu)
+cudaError_t fk_launch_fused2d_tmem(const FkGrid& g, FkOperator op, const double* Pold,
+                                   double* Pnew, int chunk0, int chunk1, int n, int N,
+                                   int sm_count, cudaStream_t s);
+cudaError_t fk_fused2d_tmem_setup(void);
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
                              int chunk0, int chunk1, cudaStream_t s);
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
