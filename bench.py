@@ -50,6 +50,18 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def load_traffic(wl_name):
+    """DRAM bytes of the dominant kernel from the committed ncu --set full capture (one launch),
+    with the algorithmic bytes of that same launch; None if there is no capture for the workload."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic_cfg3.json.txt")
+    if os.path.exists(path):
+        with open(path) as f:
+            t = json.load(f)
+        if t.get("workload") == wl_name:
+            return t
+    return None
+
+
 def coeff_table(wl):
     """(b, sigma) for all N steps as numpy [N][d][J] (autonomous: [1][d][J])."""
     if wl.autonomous:
@@ -260,6 +272,7 @@ def run_cuda(args, wl, rank, world):
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
     achieved = BYTES_PER_UPDATE * U / (dom_ms * 1e-3) / 1e9
+    tr = load_traffic(wl.name)
     h2d = int(hb.numel() * 8 + hs.numel() * 8)
     d2h = int(h_out.numel() * 8)
     return {
@@ -272,7 +285,10 @@ def run_cuda(args, wl, rank, world):
                    if (N + 1) * J * 16 > 126e6 else "state fits in L2: HBM roofline not meaningful"},
         "algorithmic_gbs": BYTES_PER_UPDATE * U / (secs / args.steps) / 1e9,
         "roofline": {"bound": "hbm", "kernel": f"fk_{dom}", "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": tr["dram_bytes"] if tr else None,
+                     "traffic_note": (f"ncu dram bytes of the launch {tr['launch']}; algorithmic bytes "
+                                      f"of that launch: {tr['algorithmic_bytes']}") if tr else None,
                      "peak_source": peak_src, "launches": dom_launches,
                      "avg_launch_ms": dom_ms / max(1, dom_launches),
                      "share_of_step": dom_ms / total_ms,
