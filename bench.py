@@ -50,6 +50,23 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def max_over_ranks(x, device=None):
+    """MAX over the ranks of the default process group (replicas: the job is as slow as its
+    slowest rank); identity when torch.distributed is not initialised."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(updates_per_replica, secs_per_step, world):
+    """Replicas only: every rank evolves the same workload; the job did world x U updates."""
+    return world * updates_per_replica / secs_per_step
+
+
 def load_traffic(wl_name):
     """DRAM bytes of the dominant kernel from the committed ncu --set full capture (one launch),
     with the algorithmic bytes of that same launch; None if there is no capture for the workload."""
@@ -230,11 +247,7 @@ def run_cuda(args, wl, rank, world):
                 fn()
             e1.record(stream)
         barrier()
-        secs = e0.elapsed_time(e1) * 1e-3
-        if world > 1:
-            t = torch.tensor([secs], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            secs = float(t.item())
+        secs = max_over_ranks(e0.elapsed_time(e1) * 1e-3, dev)
         return secs, B.fk_launch_count(ctx) - l0
 
     try:
@@ -267,7 +280,7 @@ def run_cuda(args, wl, rank, world):
         return None
     peak, peak_src = load_peaks()
     ms_step = secs / args.steps * 1e3
-    value = world * U / (secs / args.steps)
+    value = whole_job_value(U, secs / args.steps, world)
     total_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
@@ -293,7 +306,7 @@ def run_cuda(args, wl, rank, world):
                      "avg_launch_ms": dom_ms / max(1, dom_launches),
                      "share_of_step": dom_ms / total_ms,
                      "class_ms": {k: v[0] for k, v in prof.items()}},
-        "e2e": {"value": world * U / (e2e_secs / e2e_steps), "unit": UNIT,
+        "e2e": {"value": whole_job_value(U, e2e_secs / e2e_steps, world), "unit": UNIT,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_secs / e2e_steps * 1e3},
         "gpu_launches": int(launches),
