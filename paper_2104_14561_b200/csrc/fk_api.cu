@@ -269,13 +269,13 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   FK_CREATE_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
   if (p->d == 2) {                       // the fused 2-D kernel's records and step classification
     FK_CREATE_CUDA(cudaMalloc(&c->op.rec, sizeof(FkRec2) * (size_t)J));
-    FK_CREATE_CUDA(cudaMalloc(&c->d_far, sizeof(int) * (size_t)slots));
-    FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots, c->stream));
+    FK_CREATE_CUDA(cudaMalloc(&c->d_far, sizeof(int) * (size_t)slots * FK_FAR_STRIDE));
+    FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots * FK_FAR_STRIDE, c->stream));
     FK_CREATE_CUDA(fk_fused2d_setup());
     FK_CREATE_CUDA(fk_fused2d_tmem_setup());
     const char* variant = std::getenv("FK_FUSED2D");
     c->use_tmem = variant && std::strcmp(variant, "tmem") == 0;
-    c->h_far.assign(slots, 0);
+    c->h_far.assign((size_t)slots * FK_FAR_STRIDE, 0);
   }
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[0], c->n_chunks, c->stream));
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[1], c->n_chunks, c->stream));
@@ -319,9 +319,9 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
   if (c->g.d == 2) {                     // which of these steps have rows outside the fused halo
     const int s0 = step0 % c->slots;
     const int first = count < c->slots - s0 ? count : c->slots - s0;
-    FK_CUDA(c, cudaMemsetAsync(c->d_far + s0, 0, sizeof(int) * (size_t)first, c->stream));
+    FK_CUDA(c, cudaMemsetAsync(c->d_far + (size_t)s0 * FK_FAR_STRIDE, 0, sizeof(int) * (size_t)first * FK_FAR_STRIDE, c->stream));
     if (count > first)
-      FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)(count - first), c->stream));
+      FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)(count - first) * FK_FAR_STRIDE, c->stream));
     FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, step0, count, c->d_far, c->stream));
     ++c->launches;
     c->far_valid = false;
@@ -343,7 +343,7 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   std::fill(c->slot_step.begin(), c->slot_step.end(), -2);
   c->autonomous = true;
   if (c->g.d == 2) {
-    FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int), c->stream));
+    FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * FK_FAR_STRIDE, c->stream));
     FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, 0, 1, c->d_far, c->stream));
     ++c->launches;
     c->far_valid = false;
@@ -379,7 +379,7 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   const size_t slice = (size_t)c->g.d * c->g.J;
   const int last_chunk = c->N / FK_CW + 1;             // one past the chunk of column N
   if (c->g.d == 2 && !c->far_valid && n_from > n_to) { // one small read-back per coefficient load
-    FK_CUDA(c, cudaMemcpyAsync(c->h_far.data(), c->d_far, sizeof(int) * (size_t)c->slots,
+    FK_CUDA(c, cudaMemcpyAsync(c->h_far.data(), c->d_far, sizeof(int) * (size_t)c->slots * FK_FAR_STRIDE,
                                cudaMemcpyDeviceToHost, c->stream));
     FK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->far_valid = true;
@@ -402,12 +402,22 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
     double* Pnew = c->d_P[c->cur ^ 1];
     FK_LAUNCH(c, FK_K_ASSEMBLE, fk_launch_assemble(c->g, b, b + slice, c->op, c->stream));
     const bool fused = c->g.d == 2;
-    const bool generic = !fused || c->h_far[slot] > 0;   // rows the fused kernel leaves out
+    const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
+    const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
     if (fused)
       FK_LAUNCH(c, FK_K_FUSED, (c->use_tmem ? fk_launch_fused2d_tmem : fk_launch_fused2d)(c->g, c->op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
     if (generic) {
-      FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, c->stream));
-      FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, c->stream));
+      // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
+      long long sj0 = 0, sjn = c->g.J, aj0 = 0, ajn = c->g.J;
+      if (fused) {
+        const long long n1 = c->g.n[1];
+        aj0 = (long long)(FK_FAR_BIG - far[1]) * n1;
+        ajn = (long long)far[2] * n1 - aj0;
+        sj0 = (long long)(FK_FAR_BIG - far[3]) * n1;
+        sjn = (long long)far[4] * n1 - sj0;
+      }
+      FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sj0, sjn, c->stream));
+      FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, aj0, ajn, c->stream));
     }
     c->cur ^= 1;
     c->n_next = n - 1;

@@ -48,6 +48,13 @@ struct FkGrid {
 #define FK_H 2               // halo of the fused 2-D kernel (nodes per side and dimension)
 #define FK_NW (2 * FK_H + 1) // entries per dimension of a compact record
 
+// Per coefficient slot, what fk_classify finds about the rows that leave the fused halo (2-D):
+// [0] their number, [1] FK_FAR_BIG - lowest line (dimension-0 index) holding such a row,
+// [2] 1 + highest such line, [3] FK_FAR_BIG - lowest line their entries touch, [4] 1 + highest
+// line their entries touch.  All fields grow by atomicAdd / atomicMax from 0.
+#define FK_FAR_STRIDE 8
+#define FK_FAR_BIG (1 << 30)
+
 // Compact record of a near row (2-D): per dimension k the FK_NW = 2*FK_H+1 weights
 // (alpha, beta) of the nodes i_k - FK_H .. i_k + FK_H around the row's own node i_k, zero where
 // no quadrature point lands (or where the node does not exist); mask[k] has bit t set where
@@ -88,11 +95,12 @@ cudaError_t fk_launch_fused2d_tmem(const FkGrid& g, FkOperator op, const double*
                                    double* Pnew, int chunk0, int chunk1, int n, int N,
                                    int sm_count, cudaStream_t s);
 cudaError_t fk_fused2d_tmem_setup(void);
+// slopes / apply on the nodes j0 .. j0+jn-1 only (jn = J: all nodes)
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
-                             int chunk0, int chunk1, cudaStream_t s);
+                             int chunk0, int chunk1, long long j0, long long jn, cudaStream_t s);
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
                             double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
-                            int far_only, cudaStream_t s);
+                            int far_only, long long j0, long long jn, cudaStream_t s);
 cudaError_t fk_launch_gather_columns(const FkGrid& g, const double* P, int m0, int m1,
                                      double* out, cudaStream_t s);
 

@@ -170,6 +170,7 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
   const double* __restrict__ sigma = b + slice;
   long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   bool far = false;
+  int line = 0, first0 = 0, last0 = 0;
   if (j < g.J) {
     int idx[3];
     unravel(g, j, idx);
@@ -181,11 +182,19 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
         int first, last;
         fkd::reach(g, k, centre, spread, &first, &last);
         far = far || !(first >= idx[k] - FK_H && last <= idx[k] + FK_H);
+        if (k == 0) { line = idx[0]; first0 = first; last0 = last; }
       }
     }
   }
+  int* __restrict__ f = far_rows + slot * FK_FAR_STRIDE;
   const unsigned m = __ballot_sync(0xffffffffu, far);
-  if ((threadIdx.x & 31) == 0 && m) atomicAdd(far_rows + slot, __popc(m));
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(f, __popc(m));
+  if (far) {                                   // lines holding far rows, lines their entries touch
+    atomicMax(f + 1, FK_FAR_BIG - line);
+    atomicMax(f + 2, line + 1);
+    atomicMax(f + 3, FK_FAR_BIG - first0);
+    atomicMax(f + 4, last0 + 1);
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -194,9 +203,10 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
 // divided differences (R6).
 // ------------------------------------------------------------------------------------------
 __global__ void fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP,
-                          int n_chunks, int chunk0) {
+                          int n_chunks, int chunk0, long long j0, long long jn) {
   long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
-  if (j >= g.J) return;
+  if (j >= jn) return;
+  j += j0;
   const int c = chunk0 + blockIdx.y;
   int idx[3];
   unravel(g, j, idx);
@@ -237,9 +247,10 @@ template <int D>
 __global__ void __launch_bounds__(256)
 fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
          const double* __restrict__ dP, double* __restrict__ Pnew, int n_chunks, int chunk0,
-         int n, int N, int far_only) {
+         int n, int N, int far_only, long long j0, long long jn) {
   long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
-  if (j >= g.J) return;
+  if (j >= jn) return;
+  j += j0;
   const int c = chunk0 + blockIdx.y;
   const int m = c * FK_CW + threadIdx.x;
   const size_t chunk_elems = (size_t)g.J * FK_CW;
@@ -360,22 +371,22 @@ cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, i
 }
 
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
-                             int chunk0, int chunk1, cudaStream_t s) {
-  dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(chunk1 - chunk0));
-  fk_slopes<<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0);
+                             int chunk0, int chunk1, long long j0, long long jn, cudaStream_t s) {
+  dim3 block(FK_CW, 8), grid((unsigned)((jn + 7) / 8), (unsigned)(chunk1 - chunk0));
+  fk_slopes<<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0, j0, jn);
   return cudaGetLastError();
 }
 
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
                             double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
-                            int far_only, cudaStream_t s) {
-  dim3 block(FK_CW, 8), grid(node_blocks(g, 8), (unsigned)(chunk1 - chunk0));
+                            int far_only, long long j0, long long jn, cudaStream_t s) {
+  dim3 block(FK_CW, 8), grid((unsigned)((jn + 7) / 8), (unsigned)(chunk1 - chunk0));
   if (g.d == 1)
-    fk_apply<1><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only);
+    fk_apply<1><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only, j0, jn);
   else if (g.d == 2)
-    fk_apply<2><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only);
+    fk_apply<2><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only, j0, jn);
   else
-    fk_apply<3><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only);
+    fk_apply<3><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only, j0, jn);
   return cudaGetLastError();
 }
 
