@@ -37,7 +37,8 @@ constexpr int WU = W1 + 2;
 constexpr int NQ = RB + FK_NW - 1;  // union nodes of a contraction warp (8)
 constexpr int TMEM_COLS = 256;      // power of two >= LBD * NQ * 2 fields * 2 words
 constexpr size_t U_ELEMS = (size_t)LBU * WU * FK_CW;
-constexpr size_t X_ELEMS = (size_t)2 * W1 * FK_CW;   // slope exchange buffer
+constexpr size_t X_LINE = (size_t)2 * W1 * FK_CW;    // slopes of one line: [field][node][lane]
+constexpr size_t X_ELEMS = 2 * X_LINE;               // exchange buffer, two lines (by line parity)
 constexpr int NIH = W1 + 4;                          // 1/h table of the strip (dimension 1)
 constexpr size_t SMEM_BYTES = (U_ELEMS + X_ELEMS + NIH) * sizeof(double) + 2 * T1 * sizeof(FkRec2) + 48;
 static_assert(LBD * NQ * 4 <= TMEM_COLS, "slope slots must fit the TMEM allocation");
@@ -74,11 +75,10 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
 // slope warps): warp w copies the 8 nodes its partner's rows can touch (slope-window positions
 // 4w .. 4w+7) into the TMEM slot of the line: columns [4q, 4q+1] = d0, [4q+2, 4q+3] = d1.
 // Positions outside the grid stay zero (the buffer is cleared once).
-__device__ __forceinline__ void slopes_to_tmem(const FkGrid& g, const double* __restrict__ su,
+__device__ __forceinline__ void slopes_to_smem(const FkGrid& g, const double* __restrict__ su,
                                                double* __restrict__ sx,
                                                const double* __restrict__ sih, double iha,
-                                               double ihb, uint32_t tslot, int l, int s1, int w,
-                                               int lane) {
+                                               double ihb, int l, int s1, int w, int lane) {
   constexpr int NPW = W1 / NW;
   static_assert(NPW * NW == W1, "slope window must split evenly");
   const int n0 = g.n[0], n1 = g.n[1];
@@ -115,7 +115,13 @@ __device__ __forceinline__ void slopes_to_tmem(const FkGrid& g, const double* __
       sx[(W1 + p0 + k) * FK_CW + lane] = fkd::harmonic(a, b);
     }
   }
-  asm volatile("bar.sync 2, %0;" ::"n"(NW * 32) : "memory");      // slope warps only
+}
+
+// Contraction warp w copies the slopes of the 8 nodes its rows can touch (slope-window positions
+// 4w .. 4w+7) from the exchange buffer into the TMEM slot of the line: columns [4q, 4q+1] = d0,
+// [4q+2, 4q+3] = d1.  Only this warp ever reads the slot, so no cross-warp TMEM fence is needed.
+__device__ __forceinline__ void slopes_smem_to_tmem(const double* __restrict__ sx, uint32_t tslot,
+                                                    int w, int lane) {
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     double out[8];
@@ -127,6 +133,7 @@ __device__ __forceinline__ void slopes_to_tmem(const FkGrid& g, const double* __
     }
     tmem_st16(tslot + 16 * half, out);
   }
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
 __device__ __forceinline__ void u_line_copy(const FkGrid& g, const double* __restrict__ Pc,
@@ -209,17 +216,17 @@ fk_fused2d_tmem(FkGrid g, const FkRec2* __restrict__ rec, const double* __restri
         bulk_g2s(srec + (L0 & 1) * T1, rec + (size_t)L0 * n1 + s1, rec_bytes, rbar + (L0 & 1));
       }
       mbar_wait(ubar, 0);
+      // slopes of lines L0-H .. L0+H, one line per round: the slope warps fill the exchange
+      // buffer of line l while the contraction warps move line l-1 into TMEM
       const int c = max(0, L0 - H), d = min(n0, L0 + H + 1);
-      for (int l = c; l < d; ++l)
-        {
-        const int la = min(max(l - 1, 0), n0 - 3);
-        slopes_to_tmem(g, su, sx, sih, g.inv_h[0][la], g.inv_h[0][la + 1],
-                       tq + ((unsigned)l % LBD) * 32, l, s1, warp, lane);
-        asm volatile("bar.sync 2, %0;" ::"n"(NW * 32) : "memory");   // sx is reused by the next line
+      for (int l = c; l <= d; ++l) {
+        if (l < d) {
+          const int la = min(max(l - 1, 0), n0 - 3);
+          slopes_to_smem(g, su, sx + (l & 1) * X_LINE, sih, g.inv_h[0][la], g.inv_h[0][la + 1], l,
+                         s1, warp, lane);
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory");
       }
-      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory");
     }
     uint32_t uparity = 1;                                  // bit b: parity to wait for on ubar[b]
     for (int i0 = L0; i0 < L1; ++i0) {
@@ -247,12 +254,8 @@ fk_fused2d_tmem(FkGrid g, const FkRec2* __restrict__ rec, const double* __restri
           bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, rb);
         }
       }
-      if (more && ld < n0) {
-        slopes_to_tmem(g, su, sx, sih, iha, ihb, tq + ((unsigned)ld % LBD) * 32, ld, s1, warp,
-                       lane);
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-      }
-      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      if (more && ld < n0)
+        slopes_to_smem(g, su, sx + (ld & 1) * X_LINE, sih, iha, ihb, ld, s1, warp, lane);
       asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory");
     }
     return;
@@ -260,13 +263,24 @@ fk_fused2d_tmem(FkGrid g, const FkRec2* __restrict__ rec, const double* __restri
 
   // ================= contraction warps
   asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
-  asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory");     // prologue slopes are in TMEM
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  {  // prologue rounds (see the slope warps): line l-1 goes to TMEM while line l is computed
+    const int c = max(0, L0 - H), d = min(n0, L0 + H + 1);
+    for (int l = c; l <= d; ++l) {
+      if (l > c)
+        slopes_smem_to_tmem(sx + ((l - 1) & 1) * X_LINE, tq + ((unsigned)(l - 1) % LBD) * 32, warp,
+                            lane);
+      asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory");
+    }
+  }
   int ucol = (RB * warp + 1) * FK_CW + lane;
   asm volatile("" : "+r"(ucol));
   uint32_t rparity = 0;
 
   for (int i0 = L0; i0 < L1; ++i0) {
+    // slopes of line i0+H, written to the exchange buffer during iteration i0-1
+    if (i0 > L0 && i0 + H < n0)
+      slopes_smem_to_tmem(sx + ((i0 + H) & 1) * X_LINE, tq + ((unsigned)(i0 + H) % LBD) * 32, warp,
+                          lane);
     mbar_wait(rbar + (i0 & 1), (rparity >> (i0 & 1)) & 1u);
     rparity ^= 1u << (i0 & 1);
     {
@@ -332,9 +346,7 @@ fk_fused2d_tmem(FkGrid g, const FkRec2* __restrict__ rec, const double* __restri
       for (int r = 0; r < RB; ++r)
         if (store[r]) out[r * FK_CW] = acc[r];
     }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory");
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   }
   if (threadIdx.y == 0)
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tbase_smem),
