@@ -6,13 +6,16 @@
 // independent operand store (tcgen05.ld measured at > 200 B/clk/SM on B200), and its access
 // shape 32x32b (thread i of a warp <-> TMEM lane i of the warp's quarter, N consecutive
 // 32-bit columns) is exactly this library's layout: lane = output-time column.  A quarter of
-// TMEM is private to the warps with the same (warp id mod 4), so contraction warp w is paired
-// with slope warp w + 4: the slope warp computes d0 / d1 on the 8 nodes its partner's 4 rows
-// can touch and stores them with tcgen05.st; the partner fetches a whole line of them (8 nodes
-// x 2 fields) with two tcgen05.ld.x16 and gets only u through LDS.
+// TMEM is private to the warps with the same (warp id mod 4): each contraction warp keeps, in
+// its own quarter, the slopes of the 8 nodes its 4 rows can touch for the 6 resident lines.  The
+// slope warps compute every slope of the strip once into a two-line shared exchange buffer;
+// at the start of the next iteration each contraction warp moves its 8-node window of the new
+// line into TMEM (16 LDS + 2 tcgen05.st.x16), and every line body then fetches d0 / d1 with two
+// tcgen05.ld.x16 and only u through LDS (a third of the shared-memory operand traffic).
 //
 // Per block: T1 = 16 rows, 4 contraction + 4 slope warps, 256 TMEM columns (6 line slots x 32
-// columns used), shared memory only for the rolling u window and the operator records.
+// columns used), shared memory for the rolling u window, the exchange buffer and the records.
+// Selected with FK_FUSED2D=tmem; measured on par with the shared-memory variant.
 #include <cstdint>
 
 #include "fk_device.cuh"
@@ -69,12 +72,10 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
       : "memory");
 }
 
-// Slopes of line l.  Step 1: the four slope warps split the strip's W1 = 20 slope nodes, five
-// consecutive nodes each, everything in registers (as in fk_fused2d.cu), and put d0 / d1 into
-// a small shared exchange buffer sx[field][node][lane].  Step 2 (after a barrier among the
-// slope warps): warp w copies the 8 nodes its partner's rows can touch (slope-window positions
-// 4w .. 4w+7) into the TMEM slot of the line: columns [4q, 4q+1] = d0, [4q+2, 4q+3] = d1.
-// Positions outside the grid stay zero (the buffer is cleared once).
+// Slopes of line l: the four slope warps split the strip's W1 = 20 slope nodes, five consecutive
+// nodes each, everything in registers (as in fk_fused2d.cu), and put d0 / d1 into the exchange
+// buffer sx[field][node][lane] of the line.  Positions outside the grid stay zero (the buffer is
+// cleared once).
 __device__ __forceinline__ void slopes_to_smem(const FkGrid& g, const double* __restrict__ su,
                                                double* __restrict__ sx,
                                                const double* __restrict__ sih, double iha,

@@ -265,6 +265,7 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   double acc = op.c[j];
   if (D == 1) {
     double a0 = 0.0, a1 = 0.0;
+#pragma unroll 8
     for (int e = 0; e < cnt.x; ++e) {
       const double2 w0 = w[e];
       const int o = off[e];
@@ -279,6 +280,7 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
       const double2 w0 = w[e0];
       const int o0 = off[e0];
       double A = 0.0, A2 = 0.0, B0 = 0.0;
+#pragma unroll 4
       for (int e1 = 0; e1 < cnt.y; ++e1) {
         const double2 w1 = w1p[e1];
         const int o = o0 + o1p[e1];
@@ -302,6 +304,7 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
         const double2 w1 = w1p[e1];
         const int o01 = o0 + o1p[e1];
         double A = 0.0, A2 = 0.0, B0 = 0.0, B1 = 0.0;
+#pragma unroll 4
         for (int e2 = 0; e2 < cnt.z; ++e2) {
           const double2 w2 = w2p[e2];
           const int o = o01 + o2p[e2];
