@@ -130,3 +130,18 @@ def test_full_size_config_prefix_and_invariants(fk, oracle_mod, idx, nprefix):
                 assert np.all(np.take(grid, -1, axis=k) == 1.0)
     finally:
         B.fk_destroy(ctx)
+
+
+@pytest.mark.parametrize("idx", [3, 4])
+def test_tmem_variant_of_the_fused_kernel(fk, oracle_mod, idx, monkeypatch):
+    """FK_FUSED2D=tmem keeps the slopes in tensor memory (fk_fused2d_tmem.cu): same results."""
+    monkeypatch.setenv("FK_FUSED2D", "tmem")              # read by fk_create
+    wl = W.small(idx)
+    check(fk, oracle_mod, wl)
+    # full-size grid of config 3, short run: many strips, segments and chunks at once
+    if idx == 3:
+        wl = W.cellular_2d(N=70, dt=1e-3)
+        B, solve = fk
+        got = solve.evolve(wl, m0=0, m1=9)
+        ref = oracle_mod.Oracle(wl).algorithm1(8)
+        assert float(np.abs(got - ref).max()) <= TOL
