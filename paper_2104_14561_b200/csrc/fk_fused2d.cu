@@ -332,8 +332,8 @@ cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold
   const int n0 = g.n[0], n1 = g.n[1];
   const int nstrips = (n1 + T1 - 1) / T1;
   const int nchunks = chunk1 - chunk0;
-  // enough blocks for about four waves of two blocks per SM, segments of at least 16 lines
-  const long long want = 4LL * 2 * sm_count;
+  // enough blocks for about six waves of two blocks per SM, segments of at least 16 lines
+  const long long want = 6LL * 2 * sm_count;
   long long nseg = (want + (long long)nstrips * nchunks - 1) / ((long long)nstrips * nchunks);
   const int max_seg = n0 / 16 > 1 ? n0 / 16 : 1;
   if (nseg > max_seg) nseg = max_seg;

@@ -368,7 +368,7 @@ cudaError_t fk_launch_fused2d_tmem(const FkGrid& g, FkOperator op, const double*
   const int n0 = g.n[0], n1 = g.n[1];
   const int nstrips = (n1 + T1 - 1) / T1;
   const int nchunks = chunk1 - chunk0;
-  const long long want = 4LL * 2 * sm_count;
+  const long long want = 6LL * 2 * sm_count;
   long long nseg = (want + (long long)nstrips * nchunks - 1) / ((long long)nstrips * nchunks);
   const int max_seg = n0 / 16 > 1 ? n0 / 16 : 1;
   if (nseg > max_seg) nseg = max_seg;
