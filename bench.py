@@ -268,8 +268,14 @@ def run_cuda(args, wl, rank, world):
         prof = None
         if rank == 0:
             B.fk_profile(ctx, True)
-            step_device()
-            prof = B.fk_profile_read(ctx)
+            pe0 = torch.cuda.Event(enable_timing=True)
+            pe1 = torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                pe0.record(stream)
+                step_device()
+                pe1.record(stream)
+            prof = B.fk_profile_read(ctx)                   # synchronises the stream
+            prof_step_ms = pe0.elapsed_time(pe1)
             B.fk_profile(ctx, False)
             B.fk_reset(ctx)
         barrier()
@@ -281,7 +287,8 @@ def run_cuda(args, wl, rank, world):
     peak, peak_src = load_peaks()
     ms_step = secs / args.steps * 1e3
     value = whole_job_value(U, secs / args.steps, world)
-    total_ms = sum(v[0] for v in prof.values())
+    # fk_assemble runs on the library's side stream, overlapped with the previous step's
+    # kernels, so the classes do not add up to the step: shares are taken against the step time
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
     achieved = BYTES_PER_UPDATE * U / (dom_ms * 1e-3) / 1e9
@@ -304,7 +311,7 @@ def run_cuda(args, wl, rank, world):
                                       f"of that launch: {tr['algorithmic_bytes']}") if tr else None,
                      "peak_source": peak_src, "launches": dom_launches,
                      "avg_launch_ms": dom_ms / max(1, dom_launches),
-                     "share_of_step": dom_ms / total_ms,
+                     "share_of_step": dom_ms / prof_step_ms, "profiled_step_ms": prof_step_ms,
                      "class_ms": {k: v[0] for k, v in prof.items()}},
         "e2e": {"value": whole_job_value(U, e2e_secs / e2e_steps, world), "unit": UNIT,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

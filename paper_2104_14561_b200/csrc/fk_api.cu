@@ -32,7 +32,12 @@ struct fk_ctx {
   double* d_P[2] = {nullptr, nullptr};
   int cur = 0;                         // buffer holding the current state
   double* d_dP = nullptr;
-  FkOperator op = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  // the operator of step nu is assembled on a side stream while the kernels of step nu+1 run:
+  // two operator buffers (by parity of n), ready / free events between the two streams
+  FkOperator op[2] = {{nullptr, nullptr, nullptr, nullptr, nullptr},
+                      {nullptr, nullptr, nullptr, nullptr, nullptr}};
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_coef = nullptr;
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
   std::vector<int> h_far;              // host copy, valid when far_valid
   bool far_valid = false;
@@ -129,11 +134,17 @@ void release(fk_ctx* c) {
   cudaFree(c->d_P[0]);
   cudaFree(c->d_P[1]);
   cudaFree(c->d_dP);
-  cudaFree(c->op.w);
-  cudaFree(c->op.off);
-  cudaFree(c->op.cnt);
-  cudaFree(c->op.c);
-  cudaFree(c->op.rec);
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(c->op[i].w);
+    cudaFree(c->op[i].off);
+    cudaFree(c->op[i].cnt);
+    cudaFree(c->op[i].c);
+    cudaFree(c->op[i].rec);
+    if (c->ev_ready[i]) cudaEventDestroy(c->ev_ready[i]);
+    if (c->ev_free[i]) cudaEventDestroy(c->ev_free[i]);
+  }
+  if (c->ev_coef) cudaEventDestroy(c->ev_coef);
+  if (c->side) cudaStreamDestroy(c->side);
   cudaFree(c->d_far);
   cudaFree(c->d_stage);
   for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -262,13 +273,20 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   FK_CREATE_CUDA(cudaMalloc(&c->d_P[1], buf));
   FK_CREATE_CUDA(cudaMalloc(&c->d_dP, buf * p->d));
   FK_CREATE_CUDA(cudaMalloc(&c->d_coef, sizeof(double) * (size_t)slots * 2 * p->d * J));
-  FK_CREATE_CUDA(cudaMalloc(&c->op.w, sizeof(double2) * (size_t)J * g.RS));
-  FK_CREATE_CUDA(cudaMalloc(&c->op.off, sizeof(int) * (size_t)J * g.RS));
-  FK_CREATE_CUDA(cudaMalloc(&c->op.cnt, sizeof(int) * (size_t)J * 4));
-  FK_CREATE_CUDA(cudaMalloc(&c->op.c, sizeof(double) * (size_t)J));
+  FK_CREATE_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+  FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_coef, cudaEventDisableTiming));
+  for (int i = 0; i < 2; ++i) {
+    FK_CREATE_CUDA(cudaMalloc(&c->op[i].w, sizeof(double2) * (size_t)J * g.RS));
+    FK_CREATE_CUDA(cudaMalloc(&c->op[i].off, sizeof(int) * (size_t)J * g.RS));
+    FK_CREATE_CUDA(cudaMalloc(&c->op[i].cnt, sizeof(int) * (size_t)J * 4));
+    FK_CREATE_CUDA(cudaMalloc(&c->op[i].c, sizeof(double) * (size_t)J));
+    FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_ready[i], cudaEventDisableTiming));
+    FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_free[i], cudaEventDisableTiming));
+  }
   FK_CREATE_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
   if (p->d == 2) {                       // the fused 2-D kernel's records and step classification
-    FK_CREATE_CUDA(cudaMalloc(&c->op.rec, sizeof(FkRec2) * (size_t)J));
+    for (int i = 0; i < 2; ++i)
+      FK_CREATE_CUDA(cudaMalloc(&c->op[i].rec, sizeof(FkRec2) * (size_t)J));
     FK_CREATE_CUDA(cudaMalloc(&c->d_far, sizeof(int) * (size_t)slots * FK_FAR_STRIDE));
     FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots * FK_FAR_STRIDE, c->stream));
     FK_CREATE_CUDA(fk_fused2d_setup());
@@ -354,22 +372,23 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
 
 
 // one kernel launch, optionally bracketed by a pair of events of class `cls`
-#define FK_LAUNCH(c, cls_, call)                                                       \
+#define FK_LAUNCH_ON(c, stream_, cls_, call)                                           \
   do {                                                                                 \
     EventPair ep_{};                                                                   \
     if ((c)->profiling) {                                                              \
       if (!(c)->event_pool.empty()) { ep_ = (c)->event_pool.back(); (c)->event_pool.pop_back(); } \
       else { FK_CUDA(c, cudaEventCreate(&ep_.a)); FK_CUDA(c, cudaEventCreate(&ep_.b)); } \
       ep_.cls = (cls_);                                                                \
-      FK_CUDA(c, cudaEventRecord(ep_.a, (c)->stream));                                 \
+      FK_CUDA(c, cudaEventRecord(ep_.a, (stream_)));                                   \
     }                                                                                  \
     FK_CUDA(c, call);                                                                  \
     ++(c)->launches;                                                                   \
     if ((c)->profiling) {                                                              \
-      FK_CUDA(c, cudaEventRecord(ep_.b, (c)->stream));                                 \
+      FK_CUDA(c, cudaEventRecord(ep_.b, (stream_)));                                   \
       (c)->events.push_back(ep_);                                                      \
     }                                                                                  \
   } while (0)
+#define FK_LAUNCH(c, cls_, call) FK_LAUNCH_ON(c, (c)->stream, cls_, call)
 
 int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   if (!c) return FK_EINVAL;
@@ -384,6 +403,9 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
     FK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->far_valid = true;
   }
+  // the side stream must see the coefficient copies queued on the caller's stream so far
+  FK_CUDA(c, cudaEventRecord(c->ev_coef, c->stream));
+  FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_coef, 0));
   for (int n = n_from; n > n_to; --n) {
     const int nu = n - 1;
     int slot = 0;
@@ -400,12 +422,19 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
     const int chunk0 = n / FK_CW;                      // first chunk with an active column
     const double* Pold = c->d_P[c->cur];
     double* Pnew = c->d_P[c->cur ^ 1];
-    FK_LAUNCH(c, FK_K_ASSEMBLE, fk_launch_assemble(c->g, b, b + slice, c->op, c->stream));
+    // assemble A_nu into buffer n & 1 on the side stream as soon as the kernels of step n + 2
+    // (the buffer's previous users) are done; the kernels of this step wait for it
+    const int ob = n & 1;
+    const FkOperator& op = c->op[ob];
+    FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
+    FK_LAUNCH_ON(c, c->side, FK_K_ASSEMBLE, fk_launch_assemble(c->g, b, b + slice, op, c->side));
+    FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
+    FK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_ready[ob], 0));
     const bool fused = c->g.d == 2;
     const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
     const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
     if (fused)
-      FK_LAUNCH(c, FK_K_FUSED, (c->use_tmem ? fk_launch_fused2d_tmem : fk_launch_fused2d)(c->g, c->op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
+      FK_LAUNCH(c, FK_K_FUSED, (c->use_tmem ? fk_launch_fused2d_tmem : fk_launch_fused2d)(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
     if (generic) {
       // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
       long long sj0 = 0, sjn = c->g.J, aj0 = 0, ajn = c->g.J;
@@ -417,8 +446,9 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
         sjn = (long long)far[4] * n1 - sj0;
       }
       FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sj0, sjn, c->stream));
-      FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, c->op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, aj0, ajn, c->stream));
+      FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, aj0, ajn, c->stream));
     }
+    FK_CUDA(c, cudaEventRecord(c->ev_free[ob], c->stream));
     c->cur ^= 1;
     c->n_next = n - 1;
   }
