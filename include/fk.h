@@ -12,7 +12,10 @@
  * CPU fallback.  All entry points return an int code (FK_OK = 0) and never throw.  Unless a
  * parameter says otherwise the library COPIES what it is given: the caller may free or reuse
  * its buffers as soon as the call returns.  Device work is ordered on the stream given to
- * fk_create; calls on one context must not be made concurrently from several threads.
+ * fk_create (the library also owns a side stream on which it assembles the next step's operator
+ * while the current step's kernels run; it is joined to the caller's stream with events, so
+ * everything a caller can observe is ordered on the caller's stream); calls on one context must
+ * not be made concurrently from several threads.
  *
  * Index conventions.  d = dimension (1..3); n[k] nodes along dimension k; node index
  * j = ((i0*n[1])+i1)*n[2]+i2 (last dimension fastest); J = prod n[k].  Steps: dt, N,
@@ -105,7 +108,8 @@ int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem);
  * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[FK_K_COUNT]
  * and launches[FK_K_COUNT] are indexed FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY (the generic
  * slopes / apply pair) and FK_K_FUSED (the fused 2-D slopes+apply kernel).  Synchronises the
- * stream. */
+ * stream.  FK_K_ASSEMBLE is timed on the side stream, overlapped with other kernels: the classes
+ * do not add up to the duration of the step. */
 enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_FUSED = 3, FK_K_COUNT = 4 };
 int fk_profile(fk_ctx* c, int on);
 int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
