@@ -9,9 +9,11 @@
  * yields P(t_m, x_j) for every t_m in [0, T_max].
  *
  * Every step of that path runs in CUDA kernels for sm_100a inside this library; there is no
- * CPU fallback.  All entry points return an int code (FK_OK = 0) and never throw.  Unless a
- * parameter says otherwise the library COPIES what it is given: the caller may free or reuse
- * its buffers as soon as the call returns.  Device work is ordered on the stream given to
+ * CPU fallback.  All entry points return an int code (FK_OK = 0) and never throw.  The library
+ * COPIES what it is given.  A HOST buffer may be freed or reused as soon as the call returns.
+ * A DEVICE buffer (FK_MEM_DEVICE) is copied by work queued on the context's stream: it must
+ * stay valid and unmodified until that stream has reached the copy (order your own work on the
+ * same stream, or synchronise it -- fk_check does).  Device work is ordered on the stream given to
  * fk_create (the library also owns a side stream on which it assembles the next step's operator
  * while the current step's kernels run; it is joined to the caller's stream with events, so
  * everything a caller can observe is ordered on the caller's stream); calls on one context must
@@ -45,6 +47,13 @@ enum { FK_FACE_ABSORB = 0, FK_FACE_CLAMP = 1 };
 
 enum { FK_MEM_HOST = 0, FK_MEM_DEVICE = 1 };
 
+/* fk_params.flags */
+enum {
+  FK_FLAG_VALIDATE = 1   /* check every coefficient read by an updated node for NaN / Inf on the
+                            device while the operator is assembled (costs two compares per
+                            value); a hit is reported like a negative sigma, see fk_check */
+};
+
 #define FK_ALL_STEPS (-1)
 #define FK_MAX_Q 32
 
@@ -65,8 +74,9 @@ typedef struct {
   int coeff_slots;         /* number of per-step coefficient slots kept on the device:
                               N (or 0) = the full table; 1 <= s < N = a ring, step nu lives in
                               slot nu % s and must be (re)loaded before fk_evolve needs it */
-  int device;              /* CUDA device ordinal */
+  int device;              /* CUDA device ordinal (compute capability 10.x) */
   void* stream;            /* cudaStream_t (e.g. from torch); NULL = the legacy default stream */
+  unsigned flags;          /* FK_FLAG_* or 0 */
 } fk_params;
 
 /* Validate, build the Gauss-Hermite tables, allocate device state and fill both P buffers
@@ -78,9 +88,14 @@ int fk_create(const fk_params* p, fk_ctx** out);
  * sampled on the nodes at t_step: b[d][J], sigma[d][J], fp64, in host (mem = FK_MEM_HOST) or
  * device (FK_MEM_DEVICE, same device) memory.  step in 0..N-1 fills slot step % coeff_slots;
  * step = FK_ALL_STEPS declares the problem autonomous: the one slice is used by every step.
- * Values at Dirichlet nodes are never read.  sigma must be >= 0 at updated nodes (not
- * checked; a negative sigma reverses the order of the quadrature points and is undefined).
- * Copies are stream-ordered; a host buffer may be reused when the call returns. */
+ * Values at Dirichlet nodes are never read.  sigma must be >= 0 at updated nodes: a negative
+ * sigma (it would reverse the order of the quadrature points) is detected on the device when
+ * the step's operator is assembled and reported as FK_EINVAL by fk_check, by the next fk_read
+ * to host memory, or by a later fk_evolve / fk_read that finds the flag already raised; the
+ * columns computed from such a step are undefined.  Non-finite values are reported the same
+ * way when FK_FLAG_VALIDATE is set, and are undefined (they propagate as NaN) otherwise.
+ * Copies are stream-ordered; a host buffer may be reused when the call returns (the call
+ * synchronises the stream for host sources). */
 int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int mem);
 
 /* Same for `count` consecutive steps step0..step0+count-1: b and sigma are [count][d][J].
@@ -91,8 +106,12 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
 /* Algorithm 1's loop for n = n_from, n_from-1, ..., n_to+1: assemble the
  * operator nu = n-1 once and update columns n..N.  The first call after fk_create/fk_reset
  * must have n_from = N; later calls continue where the previous one stopped (n_from = its
- * n_to); after n_to = 0 all columns are final.  Asynchronous: kernels are queued on the
- * stream.  FK_ESTATE: wrong n_from, or a needed coefficient slot does not hold that step. */
+ * n_to); after n_to = 0 all columns are final.  Kernels are queued on the stream and the call
+ * returns without waiting for them, with one exception: on 2-D grids the first fk_evolve after
+ * a coefficient load synchronises the stream once to read back, per loaded step, which rows
+ * leave the fused kernel's halo (a few integers), so that the kernels of each step can be
+ * chosen on the host.  FK_ESTATE: wrong n_from, or a needed coefficient slot does not hold that
+ * step.  FK_EINVAL: a coefficient error found on the device by an earlier step (see fk_check). */
 int fk_evolve(fk_ctx* c, int n_from, int n_to);
 
 /* Refill P with chi and rewind to n = N; coefficient slots are kept. */
@@ -103,6 +122,11 @@ int fk_reset(fk_ctx* c);
  * that only column 0 and, after reaching n, nothing else is final (FK_ESTATE).  The call
  * synchronises the stream when `mem` is FK_MEM_HOST. */
 int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem);
+
+/* Synchronise the context's stream and report what the device found since the last fk_reset:
+ * FK_OK, or FK_EINVAL with fk_last_error naming the first kind of bad coefficient (negative
+ * sigma at an updated node; NaN / Inf with FK_FLAG_VALIDATE). */
+int fk_check(fk_ctx* c);
 
 /* Per-kernel-class device time of the fk_evolve calls since the last fk_reset, measured with
  * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[FK_K_COUNT]

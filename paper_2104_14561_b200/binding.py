@@ -1,8 +1,8 @@
 """ctypes binding of the C ABI in include/fk.h (libfk_b200.so): argument marshalling only.
 
 Same names as the C entry points (`fk_create`, `fk_set_coeffs`, `fk_set_coeffs_range`,
-`fk_evolve`, `fk_reset`, `fk_read`, `fk_profile`, `fk_profile_read`, `fk_launch_count`,
-`fk_destroy`, `fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
+`fk_evolve`, `fk_reset`, `fk_read`, `fk_check`, `fk_profile`, `fk_profile_read`,
+`fk_launch_count`, `fk_destroy`, `fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
 pointers) or torch CUDA tensors (device pointers); every step of the path runs in the CUDA
 kernels behind the ABI.  There is no CPU fallback: a missing library raises.
 """
@@ -18,13 +18,14 @@ FK_FACE_ABSORB, FK_FACE_CLAMP = 0, 1
 FK_MEM_HOST, FK_MEM_DEVICE = 0, 1
 FK_ALL_STEPS = -1
 FK_MAX_Q = 32
+FK_FLAG_VALIDATE = 1
 FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_COUNT = 0, 1, 2, 3, 4
 KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused")
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 
 EXPORTS = ("fk_create", "fk_set_coeffs", "fk_set_coeffs_range", "fk_evolve", "fk_reset",
-           "fk_read", "fk_profile", "fk_profile_read", "fk_launch_count", "fk_destroy",
+           "fk_read", "fk_check", "fk_profile", "fk_profile_read", "fk_launch_count", "fk_destroy",
            "fk_last_error", "fk_gauss_hermite")
 
 
@@ -38,7 +39,8 @@ class fk_params(C.Structure):
     _fields_ = [("d", C.c_int), ("n", C.c_int * 3), ("x", C.POINTER(C.c_double) * 3),
                 ("dt", C.c_double), ("N", C.c_int), ("Q", C.c_int * 3),
                 ("face_kind", (C.c_int * 2) * 3), ("face_value", (C.c_double * 2) * 3),
-                ("coeff_slots", C.c_int), ("device", C.c_int), ("stream", C.c_void_p)]
+                ("coeff_slots", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
+                ("flags", C.c_uint)]
 
 
 _lib = None
@@ -60,6 +62,7 @@ def lib():
         L.fk_evolve.argtypes = [vp, C.c_int, C.c_int]
         L.fk_reset.argtypes = [vp]
         L.fk_read.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
+        L.fk_check.argtypes = [vp]
         L.fk_profile.argtypes = [vp, C.c_int]
         L.fk_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.fk_launch_count.argtypes = [vp]
@@ -103,7 +106,7 @@ def fk_gauss_hermite(Q):
     return a, w
 
 
-def fk_create(x, dt, N, Q, face_kind, face_value, coeff_slots=0, device=0, stream=0):
+def fk_create(x, dt, N, Q, face_kind, face_value, coeff_slots=0, device=0, stream=0, flags=0):
     """-> opaque context handle.  x: list of d node arrays; Q, face_kind[d][2], face_value[d][2]."""
     p = fk_params()
     d = len(x)
@@ -123,6 +126,7 @@ def fk_create(x, dt, N, Q, face_kind, face_value, coeff_slots=0, device=0, strea
     p.coeff_slots = int(coeff_slots)
     p.device = int(device)
     p.stream = C.c_void_p(int(stream) or None)
+    p.flags = int(flags)
     ctx = C.c_void_p()
     rc = lib().fk_create(C.byref(p), C.byref(ctx))
     if rc != FK_OK:
@@ -161,6 +165,11 @@ def fk_read(ctx, m0, m1, out):
         raise TypeError("out must be a C-contiguous float64 numpy array or torch tensor")
     _check(ctx, lib().fk_read(ctx, int(m0), int(m1), po, mo))
     return out
+
+
+def fk_check(ctx):
+    """Synchronise the stream; raise FkError(FK_EINVAL) if the device found a bad coefficient."""
+    _check(ctx, lib().fk_check(ctx))
 
 
 def fk_profile(ctx, on):

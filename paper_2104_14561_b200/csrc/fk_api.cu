@@ -38,11 +38,12 @@ struct fk_ctx {
                       {nullptr, nullptr, nullptr, nullptr, nullptr}};
   cudaStream_t side = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_coef = nullptr;
+  int* d_status = nullptr;             // device status word: FK_BAD_* bits raised by fk_assemble
+  int* h_status = nullptr;             // pinned host copy, refreshed at the end of every fk_evolve
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
   std::vector<int> h_far;              // host copy, valid when far_valid
   bool far_valid = false;
   int sm_count = 148;
-  bool use_tmem = false;               // fused 2-D variant: slopes in smem; FK_FUSED2D=tmem: in TMEM
   double* d_stage = nullptr;           // fk_read staging for host destinations
   size_t stage_bytes = 0;
   int n_next = 0;                      // the n the next fk_evolve must start from
@@ -64,6 +65,16 @@ int cuda_fail(fk_ctx* c, cudaError_t e, const char* what) {
   return fail(c, e == cudaErrorMemoryAllocation ? FK_ENOMEM : FK_ECUDA,
               std::string(what) + ": " + cudaGetErrorString(e));
 }
+
+// every entry point runs on the context's device and leaves the caller's current device alone
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) cudaSetDevice(dev);
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 #define FK_CUDA(c, call)                                       \
   do {                                                         \
@@ -128,7 +139,7 @@ void gauss_hermite(int Q, double* a, double* w) {
 
 void release(fk_ctx* c) {
   if (!c) return;
-  cudaSetDevice(c->device);
+  DeviceGuard guard(c->device);
   for (int k = 0; k < 3; ++k) { cudaFree(c->d_x[k]); cudaFree(c->d_invh[k]); }
   cudaFree(c->d_coef);
   cudaFree(c->d_P[0]);
@@ -146,6 +157,8 @@ void release(fk_ctx* c) {
   if (c->ev_coef) cudaEventDestroy(c->ev_coef);
   if (c->side) cudaStreamDestroy(c->side);
   cudaFree(c->d_far);
+  cudaFree(c->d_status);
+  if (c->h_status) cudaFreeHost(c->h_status);
   cudaFree(c->d_stage);
   for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   for (auto& e : c->event_pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -203,6 +216,12 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
     return fail(nullptr, FK_ECUDA, "no CUDA device: this library has no CPU path");
   if (p->device < 0 || p->device >= ndev) return fail(nullptr, FK_EINVAL, "bad device ordinal");
+  int cc_major = 0;
+  if (cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, p->device) != cudaSuccess ||
+      cc_major != 10)
+    return fail(nullptr, FK_ECUDA, "device is not compute capability 10.x: the kernels are built for sm_100a only");
+  if (p->flags & ~(unsigned)FK_FLAG_VALIDATE) return fail(nullptr, FK_EINVAL, "unknown bits in flags");
+  DeviceGuard guard(p->device);
 
   fk_ctx* c = new (std::nothrow) fk_ctx();
   if (!c) return fail(nullptr, FK_ENOMEM, "host allocation failed");
@@ -220,6 +239,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   g.J = J;
   g.dt = p->dt;
   g.sq = std::sqrt(2.0 * p->dt);
+  g.validate = (p->flags & FK_FLAG_VALIDATE) ? 1 : 0;
   int qoff = 0;
   for (int k = 0; k < 3; ++k) { g.n[k] = 1; g.Q[k] = 0; g.stride[k] = 0; }
   long long st = 1;
@@ -255,7 +275,6 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     }                                                                           \
   } while (0)
 
-  FK_CREATE_CUDA(cudaSetDevice(c->device));
   for (int k = 0; k < p->d; ++k) {
     const int n = p->n[k];
     std::vector<double> ih(n - 1);
@@ -283,16 +302,19 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_ready[i], cudaEventDisableTiming));
     FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_free[i], cudaEventDisableTiming));
   }
+  FK_CREATE_CUDA(cudaMalloc(&c->d_status, sizeof(int)));
+  FK_CREATE_CUDA(cudaMemsetAsync(c->d_status, 0, sizeof(int), c->stream));
+  FK_CREATE_CUDA(cudaHostAlloc(&c->h_status, sizeof(int), cudaHostAllocDefault));
+  *c->h_status = 0;
   FK_CREATE_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
   if (p->d == 2) {                       // the fused 2-D kernel's records and step classification
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < 2; ++i) {
       FK_CREATE_CUDA(cudaMalloc(&c->op[i].rec, sizeof(FkRec2) * (size_t)J));
+      FK_CREATE_CUDA(cudaMemsetAsync(c->op[i].rec, 0, sizeof(FkRec2) * (size_t)J, c->stream));
+    }
     FK_CREATE_CUDA(cudaMalloc(&c->d_far, sizeof(int) * (size_t)slots * FK_FAR_STRIDE));
     FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots * FK_FAR_STRIDE, c->stream));
     FK_CREATE_CUDA(fk_fused2d_setup());
-    FK_CREATE_CUDA(fk_fused2d_tmem_setup());
-    const char* variant = std::getenv("FK_FUSED2D");
-    c->use_tmem = variant && std::strcmp(variant, "tmem") == 0;
     c->h_far.assign((size_t)slots * FK_FAR_STRIDE, 0);
   }
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[0], c->n_chunks, c->stream));
@@ -305,10 +327,12 @@ int fk_create(const fk_params* p, fk_ctx** out) {
 
 int fk_reset(fk_ctx* c) {
   if (!c) return FK_EINVAL;
-  FK_CUDA(c, cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   FK_CUDA(c, fk_launch_fill_chi(c->g, c->d_P[0], c->n_chunks, c->stream));
   FK_CUDA(c, fk_launch_fill_chi(c->g, c->d_P[1], c->n_chunks, c->stream));
   c->launches += 2;
+  FK_CUDA(c, cudaMemsetAsync(c->d_status, 0, sizeof(int), c->stream));
+  *c->h_status = 0;
   c->cur = 0;
   c->n_next = c->N;
   for (auto& e : c->events) c->event_pool.push_back(e);
@@ -323,7 +347,7 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
   if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
   if (count < 1 || count > c->slots) return fail(c, FK_EINVAL, "count must be 1..coeff_slots");
   if (step0 < 0 || step0 + count > c->N) return fail(c, FK_EINVAL, "step range outside 0..N-1");
-  FK_CUDA(c, cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   const size_t slice = (size_t)c->g.d * c->g.J;      // doubles per [d][J] array
   const cudaMemcpyKind kind = mem == FK_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
   for (int i = 0; i < count; ++i) {
@@ -353,7 +377,7 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   if (step != FK_ALL_STEPS) return fk_set_coeffs_range(c, step, 1, b, sigma, mem);
   if (!b || !sigma) return fail(c, FK_EINVAL, "b or sigma is NULL");
   if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
-  FK_CUDA(c, cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   const size_t slice = (size_t)c->g.d * c->g.J;
   const cudaMemcpyKind kind = mem == FK_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
   FK_CUDA(c, cudaMemcpyAsync(c->d_coef, b, sizeof(double) * slice, kind, c->stream));
@@ -371,32 +395,110 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
 }
 
 
-// one kernel launch, optionally bracketed by a pair of events of class `cls`
-#define FK_LAUNCH_ON(c, stream_, cls_, call)                                           \
-  do {                                                                                 \
-    EventPair ep_{};                                                                   \
-    if ((c)->profiling) {                                                              \
-      if (!(c)->event_pool.empty()) { ep_ = (c)->event_pool.back(); (c)->event_pool.pop_back(); } \
-      else { FK_CUDA(c, cudaEventCreate(&ep_.a)); FK_CUDA(c, cudaEventCreate(&ep_.b)); } \
-      ep_.cls = (cls_);                                                                \
-      FK_CUDA(c, cudaEventRecord(ep_.a, (stream_)));                                   \
-    }                                                                                  \
-    FK_CUDA(c, call);                                                                  \
-    ++(c)->launches;                                                                   \
-    if ((c)->profiling) {                                                              \
-      FK_CUDA(c, cudaEventRecord(ep_.b, (stream_)));                                   \
-      (c)->events.push_back(ep_);                                                      \
-    }                                                                                  \
-  } while (0)
-#define FK_LAUNCH(c, cls_, call) FK_LAUNCH_ON(c, (c)->stream, cls_, call)
+}  // extern "C"
+
+namespace {
+
+// one kernel launch, optionally bracketed by a pair of events of class `cls`; the pair goes
+// back to the pool when the launch fails
+template <class Launch>
+int launch_on(fk_ctx* c, cudaStream_t st, int cls, const char* what, Launch&& launch) {
+  EventPair ep{};
+  if (c->profiling) {
+    if (!c->event_pool.empty()) { ep = c->event_pool.back(); c->event_pool.pop_back(); }
+    else { FK_CUDA(c, cudaEventCreate(&ep.a)); FK_CUDA(c, cudaEventCreate(&ep.b)); }
+    ep.cls = cls;
+  }
+  cudaError_t e = c->profiling ? cudaEventRecord(ep.a, st) : cudaSuccess;
+  if (e == cudaSuccess) e = launch();
+  if (e == cudaSuccess && c->profiling) e = cudaEventRecord(ep.b, st);
+  if (e != cudaSuccess) {
+    if (c->profiling) c->event_pool.push_back(ep);
+    return cuda_fail(c, e, what);
+  }
+  ++c->launches;
+  if (c->profiling) c->events.push_back(ep);
+  return FK_OK;
+}
+#define FK_TRY(expr) do { int rc_ = (expr); if (rc_ != FK_OK) return rc_; } while (0)
+
+const char* status_text(int bits) {
+  if (bits & FK_BAD_NEG_SIGMA) return "negative sigma at an updated node (found on the device while assembling a step operator)";
+  if (bits & FK_BAD_NONFINITE) return "NaN or Inf coefficient at an updated node (FK_FLAG_VALIDATE)";
+  return "";
+}
+
+// one step of Algorithm 1: assemble A_nu (nu = n-1) on the side stream,
+// update columns n..N on the caller's stream
+int evolve_step(fk_ctx* c, int n) {
+  const size_t slice = (size_t)c->g.d * c->g.J;
+  const int last_chunk = c->N / FK_CW + 1;             // one past the chunk of column N
+  const int nu = n - 1;
+  int slot = 0;
+  if (!c->autonomous) {
+    slot = nu % c->slots;
+    if (c->slot_step[slot] != nu) {
+      char msg[96];
+      std::snprintf(msg, sizeof msg, "coefficients of step %d are not loaded", nu);
+      return fail(c, FK_ESTATE, msg);
+    }
+  }
+  const double* b = c->d_coef + (size_t)slot * 2 * slice;
+  const int chunk0 = n / FK_CW;                        // first chunk with an active column
+  const double* Pold = c->d_P[c->cur];
+  double* Pnew = c->d_P[c->cur ^ 1];
+  // assemble A_nu into buffer n & 1 on the side stream as soon as the kernels of step n + 2
+  // (the buffer's previous users) are done; the kernels of this step wait for it
+  const int ob = n & 1;
+  const FkOperator& op = c->op[ob];
+  cudaStream_t st = c->stream;
+  FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
+  FK_TRY(launch_on(c, c->side, FK_K_ASSEMBLE, "fk_assemble", [&] {
+    return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->side); }));
+  FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
+  FK_CUDA(c, cudaStreamWaitEvent(st, c->ev_ready[ob], 0));
+  const bool fused = c->g.d == 2;
+  const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
+  const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
+  if (fused)
+    FK_TRY(launch_on(c, st, FK_K_FUSED, "fk_fused2d", [&] {
+      return fk_launch_fused2d(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, st); }));
+  if (generic) {
+    // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
+    long long sj0 = 0, sjn = c->g.J, aj0 = 0, ajn = c->g.J;
+    if (fused) {
+      const long long n1 = c->g.n[1];
+      aj0 = (long long)(FK_FAR_BIG - far[1]) * n1;
+      ajn = (long long)far[2] * n1 - aj0;
+      sj0 = (long long)(FK_FAR_BIG - far[3]) * n1;
+      sjn = (long long)far[4] * n1 - sj0;
+    }
+    FK_TRY(launch_on(c, st, FK_K_SLOPES, "fk_slopes", [&] {
+      return fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sj0, sjn, st); }));
+    FK_TRY(launch_on(c, st, FK_K_APPLY, "fk_apply", [&] {
+      return fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
+                             fused ? 1 : 0, aj0, ajn, st); }));
+  }
+  FK_CUDA(c, cudaEventRecord(c->ev_free[ob], st));
+  return FK_OK;
+}
+
+// after a failure inside a step: make the caller's stream wait for whatever the side stream
+// still has queued, so that the two never run unordered past the failing call (best effort)
+void join_side(fk_ctx* c) {
+  if (cudaEventRecord(c->ev_coef, c->side) == cudaSuccess) cudaStreamWaitEvent(c->stream, c->ev_coef, 0);
+}
+
+}  // namespace
+
+extern "C" {
 
 int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   if (!c) return FK_EINVAL;
   if (n_from != c->n_next) return fail(c, FK_ESTATE, "n_from must continue where the last fk_evolve stopped (N after create/reset)");
   if (n_to < 0 || n_to > n_from) return fail(c, FK_EINVAL, "need 0 <= n_to <= n_from");
-  FK_CUDA(c, cudaSetDevice(c->device));
-  const size_t slice = (size_t)c->g.d * c->g.J;
-  const int last_chunk = c->N / FK_CW + 1;             // one past the chunk of column N
+  if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
+  DeviceGuard guard(c->device);
   if (c->g.d == 2 && !c->far_valid && n_from > n_to) { // one small read-back per coefficient load
     FK_CUDA(c, cudaMemcpyAsync(c->h_far.data(), c->d_far, sizeof(int) * (size_t)c->slots * FK_FAR_STRIDE,
                                cudaMemcpyDeviceToHost, c->stream));
@@ -407,51 +509,26 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   FK_CUDA(c, cudaEventRecord(c->ev_coef, c->stream));
   FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_coef, 0));
   for (int n = n_from; n > n_to; --n) {
-    const int nu = n - 1;
-    int slot = 0;
-    if (!c->autonomous) {
-      slot = nu % c->slots;
-      if (c->slot_step[slot] != nu) {
-        c->n_next = n;
-        char msg[96];
-        std::snprintf(msg, sizeof msg, "coefficients of step %d are not loaded", nu);
-        return fail(c, FK_ESTATE, msg);
-      }
+    const int rc = evolve_step(c, n);
+    if (rc != FK_OK) {
+      join_side(c);
+      c->n_next = n;                 // the step was not completed; P still holds the state of n
+      return rc;
     }
-    const double* b = c->d_coef + (size_t)slot * 2 * slice;
-    const int chunk0 = n / FK_CW;                      // first chunk with an active column
-    const double* Pold = c->d_P[c->cur];
-    double* Pnew = c->d_P[c->cur ^ 1];
-    // assemble A_nu into buffer n & 1 on the side stream as soon as the kernels of step n + 2
-    // (the buffer's previous users) are done; the kernels of this step wait for it
-    const int ob = n & 1;
-    const FkOperator& op = c->op[ob];
-    FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
-    FK_LAUNCH_ON(c, c->side, FK_K_ASSEMBLE, fk_launch_assemble(c->g, b, b + slice, op, c->side));
-    FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
-    FK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_ready[ob], 0));
-    const bool fused = c->g.d == 2;
-    const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
-    const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
-    if (fused)
-      FK_LAUNCH(c, FK_K_FUSED, (c->use_tmem ? fk_launch_fused2d_tmem : fk_launch_fused2d)(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, c->stream));
-    if (generic) {
-      // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
-      long long sj0 = 0, sjn = c->g.J, aj0 = 0, ajn = c->g.J;
-      if (fused) {
-        const long long n1 = c->g.n[1];
-        aj0 = (long long)(FK_FAR_BIG - far[1]) * n1;
-        ajn = (long long)far[2] * n1 - aj0;
-        sj0 = (long long)(FK_FAR_BIG - far[3]) * n1;
-        sjn = (long long)far[4] * n1 - sj0;
-      }
-      FK_LAUNCH(c, FK_K_SLOPES, fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sj0, sjn, c->stream));
-      FK_LAUNCH(c, FK_K_APPLY, fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N, fused ? 1 : 0, aj0, ajn, c->stream));
-    }
-    FK_CUDA(c, cudaEventRecord(c->ev_free[ob], c->stream));
     c->cur ^= 1;
     c->n_next = n - 1;
   }
+  if (n_from > n_to)                 // refresh the host copy of the device status word
+    FK_CUDA(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  return FK_OK;
+}
+
+int fk_check(fk_ctx* c) {
+  if (!c) return FK_EINVAL;
+  DeviceGuard guard(c->device);
+  FK_CUDA(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
   return FK_OK;
 }
 
@@ -461,7 +538,8 @@ int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem) {
   if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
   if (m0 < 0 || m1 > c->N + 1 || m0 >= m1) return fail(c, FK_EINVAL, "need 0 <= m0 < m1 <= N+1");
   if (c->n_next != 0 && m1 > 1) return fail(c, FK_ESTATE, "columns other than 0 are final only after fk_evolve reached n_to = 0");
-  FK_CUDA(c, cudaSetDevice(c->device));
+  if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
+  DeviceGuard guard(c->device);
   const double* P = c->d_P[c->cur];
   const size_t col = sizeof(double) * (size_t)c->g.J;
   if (mem == FK_MEM_DEVICE) {
@@ -490,6 +568,7 @@ int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem) {
                                cudaMemcpyDeviceToHost, c->stream));
     FK_CUDA(c, cudaStreamSynchronize(c->stream));
   }
+  if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));   // refreshed by fk_evolve
   return FK_OK;
 }
 
@@ -502,7 +581,7 @@ int fk_profile(fk_ctx* c, int on) {
 int fk_profile_read(fk_ctx* c, double* ms, long long* launches) {
   if (!c) return FK_EINVAL;
   if (!ms || !launches) return fail(c, FK_EINVAL, "ms or launches is NULL");
-  FK_CUDA(c, cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   FK_CUDA(c, cudaStreamSynchronize(c->stream));
   for (int k = 0; k < FK_K_COUNT; ++k) { ms[k] = 0.0; launches[k] = 0; }
   for (auto& e : c->events) {

@@ -34,11 +34,16 @@ struct FkGrid {
   double lo[3], hi[3];    // box faces = x[k][0], x[k][n-1]
   double inv_h0[3];       // (n-1)/(hi-lo)
   double dt, sq;          // sq = sqrt(2 dt)
+  int validate;           // FK_FLAG_VALIDATE: report NaN / Inf coefficients of updated nodes
   const double* x[3];     // device: node coordinates
   const double* inv_h[3]; // device: 1/(x[i+1]-x[i]), n-1 values
   double gh_a[3][FK_QMAX];
   double gh_w[3][FK_QMAX];
 };
+
+// bits of the device status word (coefficient errors found by fk_assemble)
+#define FK_BAD_NEG_SIGMA 1
+#define FK_BAD_NONFINITE 2
 
 // Row flags kept in cnt[j][3]
 #define FK_ROW_DIRICHLET 1   // node on an ABSORB face: the row is the constant c_j = g
@@ -78,7 +83,7 @@ struct FkOperator {       // device pointers of one assembled A_nu
 // launchers (fk_kernels.cu); all asynchronous on `s`, return the launch's cudaError_t
 cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStream_t s);
 cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
-                               FkOperator op, cudaStream_t s);
+                               FkOperator op, int* status, cudaStream_t s);
 // far_rows[slot] = number of rows of the step held in that coefficient slot that are not
 // FK_ROW_NEAR (2-D only), for the `count` steps step0.. whose slices sit at
 // coef + (step % slots) * 2*d*J (b then sigma); far_rows entries must be zeroed before
@@ -90,11 +95,6 @@ cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold
                               int chunk0, int chunk1, int n, int N, int sm_count,
                               cudaStream_t s);
 cudaError_t fk_fused2d_setup(void);
-// same contract, slopes kept in tensor memory instead of shared memory (fk_fused2d_tmem.cu)
-cudaError_t fk_launch_fused2d_tmem(const FkGrid& g, FkOperator op, const double* Pold,
-                                   double* Pnew, int chunk0, int chunk1, int n, int N,
-                                   int sm_count, cudaStream_t s);
-cudaError_t fk_fused2d_tmem_setup(void);
 // slopes / apply on the nodes j0 .. j0+jn-1 only (jn = J: all nodes)
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
                              int chunk0, int chunk1, long long j0, long long jn, cudaStream_t s);

@@ -49,7 +49,8 @@ __global__ void fk_fill_chi(FkGrid g, double* __restrict__ P, int n_chunks) {
 // around it per dimension, zero where no point lands.
 // ------------------------------------------------------------------------------------------
 __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
-                            const double* __restrict__ sigma, FkOperator op) {
+                            const double* __restrict__ sigma, FkOperator op,
+                            int* __restrict__ status) {
   long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= g.J) return;
   int idx[3];
@@ -65,6 +66,10 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
       rec->c = gval;
       rec->mask[0] = rec->mask[1] = 0;
       rec->flags = FK_ROW_DIRICHLET;
+      // the fused kernel multiplies every slot of the rows it owns: the weights of a Dirichlet
+      // row must be zeros, not whatever the allocation held
+      for (int k = 0; k < 2; ++k)
+        for (int e = 0; e < FK_NW; ++e) rec->w[k][e] = make_double2(0.0, 0.0);
     }
     return;
   }
@@ -72,10 +77,14 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
   int* __restrict__ rowo = op.off + (size_t)j * g.RS;
   double cj = 0.0, mass = 1.0;
   bool near = rec != nullptr;
+  int bad = 0;
   for (int k = 0; k < g.d; ++k) {
     const double xk = g.x[k][idx[k]];
-    const double centre = __dadd_rn(xk, __dmul_rn(b[(size_t)k * g.J + j], g.dt));
-    const double spread = __dmul_rn(sigma[(size_t)k * g.J + j], g.sq);
+    const double bk = b[(size_t)k * g.J + j], sk = sigma[(size_t)k * g.J + j];
+    if (sk < 0.0) bad |= FK_BAD_NEG_SIGMA;
+    if (g.validate && !(isfinite(bk) && isfinite(sk))) bad |= FK_BAD_NONFINITE;
+    const double centre = __dadd_rn(xk, __dmul_rn(bk, g.dt));
+    const double spread = __dmul_rn(sk, g.sq);
     const double lo = g.lo[k], hi = g.hi[k];
     const long long unit = g.stride[k] * FK_CW;
     bool rec_k = false;
@@ -149,6 +158,7 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
     cj += mass * ek;
     mass *= mk;
   }
+  if (bad) atomicOr(status, bad);
   for (int k = g.d; k < 3; ++k) cnt[k] = 0;
   cnt[3] = near ? FK_ROW_NEAR : 0;
   op.c[j] = cj;
@@ -160,40 +170,46 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
 
 // ------------------------------------------------------------------------------------------
 // fk_classify (2-D): how many rows of each loaded step are not FK_ROW_NEAR, by the same
-// fkd::reach test fk_assemble applies.  grid = (node blocks, steps); one atomic per warp.
+// fkd::reach test fk_assemble applies.  grid = (node blocks, min(steps, 4096)).
 // ------------------------------------------------------------------------------------------
 __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots, int step0,
-                            int* __restrict__ far_rows) {
-  const int slot = (step0 + (int)blockIdx.y) % slots;
+                            int count, int* __restrict__ far_rows) {
   const size_t slice = (size_t)g.d * g.J;
-  const double* __restrict__ b = coef + (size_t)slot * 2 * slice;
-  const double* __restrict__ sigma = b + slice;
-  long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  bool far = false;
-  int line = 0, first0 = 0, last0 = 0;
-  if (j < g.J) {
-    int idx[3];
-    unravel(g, j, idx);
-    double gval;
-    if (!dirichlet(g, idx, &gval)) {
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int idx[3] = {0, 0, 0};
+  double gval;
+  const bool updated = j < g.J && (unravel(g, j, idx), !dirichlet(g, idx, &gval));
+  for (int s = blockIdx.y; s < count; s += gridDim.y) {      // any number of steps per launch
+    const int slot = (step0 + s) % slots;
+    const double* __restrict__ b = coef + (size_t)slot * 2 * slice;
+    const double* __restrict__ sigma = b + slice;
+    bool far = false;
+    int first0 = 0, last0 = 0;
+    if (updated) {
       for (int k = 0; k < g.d; ++k) {
         const double centre = __dadd_rn(g.x[k][idx[k]], __dmul_rn(b[(size_t)k * g.J + j], g.dt));
         const double spread = __dmul_rn(sigma[(size_t)k * g.J + j], g.sq);
         int first, last;
         fkd::reach(g, k, centre, spread, &first, &last);
         far = far || !(first >= idx[k] - FK_H && last <= idx[k] + FK_H);
-        if (k == 0) { line = idx[0]; first0 = first; last0 = last; }
+        if (k == 0) { first0 = first; last0 = last; }
       }
     }
-  }
-  int* __restrict__ f = far_rows + slot * FK_FAR_STRIDE;
-  const unsigned m = __ballot_sync(0xffffffffu, far);
-  if ((threadIdx.x & 31) == 0 && m) atomicAdd(f, __popc(m));
-  if (far) {                                   // lines holding far rows, lines their entries touch
-    atomicMax(f + 1, FK_FAR_BIG - line);
-    atomicMax(f + 2, line + 1);
-    atomicMax(f + 3, FK_FAR_BIG - first0);
-    atomicMax(f + 4, last0 + 1);
+    int* __restrict__ f = far_rows + slot * FK_FAR_STRIDE;
+    const unsigned m = __ballot_sync(0xffffffffu, far);
+    if (m) {                                  // one set of atomics per warp that holds far rows
+      const int a1 = __reduce_max_sync(0xffffffffu, far ? FK_FAR_BIG - idx[0] : 0);
+      const int a2 = __reduce_max_sync(0xffffffffu, far ? idx[0] + 1 : 0);
+      const int a3 = __reduce_max_sync(0xffffffffu, far ? FK_FAR_BIG - first0 : 0);
+      const int a4 = __reduce_max_sync(0xffffffffu, far ? last0 + 1 : 0);
+      if ((threadIdx.x & 31) == 0) {
+        atomicAdd(f, __popc(m));
+        atomicMax(f + 1, a1);                 // lines holding far rows, lines their entries touch
+        atomicMax(f + 2, a2);
+        atomicMax(f + 3, a3);
+        atomicMax(f + 4, a4);
+      }
+    }
   }
 }
 
@@ -361,15 +377,15 @@ cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStr
 }
 
 cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
-                               FkOperator op, cudaStream_t s) {
-  fk_assemble<<<node_blocks(g, 128), 128, 0, s>>>(g, b, sigma, op);
+                               FkOperator op, int* status, cudaStream_t s) {
+  fk_assemble<<<node_blocks(g, 128), 128, 0, s>>>(g, b, sigma, op, status);
   return cudaGetLastError();
 }
 
 cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, int step0,
                                int count, int* far_rows, cudaStream_t s) {
-  dim3 grid(node_blocks(g, 128), (unsigned)count);
-  fk_classify<<<grid, 128, 0, s>>>(g, coef, slots, step0, far_rows);
+  dim3 grid(node_blocks(g, 128), (unsigned)(count < 4096 ? count : 4096));
+  fk_classify<<<grid, 128, 0, s>>>(g, coef, slots, step0, count, far_rows);
   return cudaGetLastError();
 }
 

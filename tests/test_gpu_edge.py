@@ -132,16 +132,75 @@ def test_full_size_config_prefix_and_invariants(fk, oracle_mod, idx, nprefix):
         B.fk_destroy(ctx)
 
 
-@pytest.mark.parametrize("idx", [3, 4])
-def test_tmem_variant_of_the_fused_kernel(fk, oracle_mod, idx, monkeypatch):
-    """FK_FUSED2D=tmem keeps the slopes in tensor memory (fk_fused2d_tmem.cu): same results."""
-    monkeypatch.setenv("FK_FUSED2D", "tmem")              # read by fk_create
-    wl = W.small(idx)
-    check(fk, oracle_mod, wl)
-    # full-size grid of config 3, short run: many strips, segments and chunks at once
-    if idx == 3:
-        wl = W.cellular_2d(N=70, dt=1e-3)
-        B, solve = fk
-        got = solve.evolve(wl, m0=0, m1=9)
-        ref = oracle_mod.Oracle(wl).algorithm1(8)
+def test_negative_sigma_and_nonfinite_coefficients_are_reported(fk):
+    """negative sigma is FK_EINVAL; NaN / Inf only with the validate flag."""
+    B, solve = fk
+    for idx in (2, 3, 5):                                   # 1-D, 2-D (fused kernel), 3-D
+        wl = W.small(idx)
+        b, s = wl.coeff_table(0, wl.N)
+        interior = wl.J // 2 + 1                            # not on a face in any of the shapes
+        # (1) negative sigma at an updated node of one step
+        s_bad = s.copy()
+        s_bad[3, 0, interior] = -0.1
+        ctx = solve.create_for(wl, wl.N)
+        try:
+            B.fk_set_coeffs_range(ctx, 0, wl.N, b, s_bad)
+            B.fk_evolve(ctx, wl.N, 0)                       # queued; the flag is raised on the device
+            with pytest.raises(B.FkError) as e:
+                B.fk_check(ctx)
+            assert e.value.code == B.FK_EINVAL and "negative sigma" in str(e.value)
+            with pytest.raises(B.FkError) as e:
+                B.fk_read(ctx, 0, wl.N + 1, np.empty((wl.N + 1, wl.J)))
+            assert e.value.code == B.FK_EINVAL
+            # good coefficients + fk_reset clear it
+            B.fk_reset(ctx)
+            B.fk_set_coeffs_range(ctx, 0, wl.N, b, s)
+            B.fk_evolve(ctx, wl.N, 0)
+            B.fk_check(ctx)
+        finally:
+            B.fk_destroy(ctx)
+        # (2) a negative sigma on a Dirichlet node is never read
+        s_ok = s.copy()
+        s_ok[:, :, 0] = -1.0                                # node 0 lies on an ABSORB face in all three
+        ctx = solve.create_for(wl, wl.N)
+        try:
+            B.fk_set_coeffs_range(ctx, 0, wl.N, b, s_ok)
+            B.fk_evolve(ctx, wl.N, 0)
+            B.fk_check(ctx)
+        finally:
+            B.fk_destroy(ctx)
+        # (3) NaN drift: reported only with FK_FLAG_VALIDATE
+        b_nan = b.copy()
+        b_nan[1, 0, interior] = np.nan
+        for flags, raises in ((B.FK_FLAG_VALIDATE, True), (0, False)):
+            ctx = solve.create_for(wl, wl.N, flags=flags)
+            try:
+                B.fk_set_coeffs_range(ctx, 0, wl.N, b_nan, s)
+                B.fk_evolve(ctx, wl.N, 0)
+                if raises:
+                    with pytest.raises(B.FkError) as e:
+                        B.fk_check(ctx)
+                    assert e.value.code == B.FK_EINVAL and "NaN" in str(e.value)
+                else:
+                    B.fk_check(ctx)
+            finally:
+                B.fk_destroy(ctx)
+
+
+def test_results_do_not_depend_on_what_freed_device_memory_held(fk, oracle_mod):
+    """Operator buffers come from plain cudaMalloc: poison freed device memory with NaN patterns
+    first; Dirichlet rows (g != 1 faces) and every padded slot must still be exact."""
+    import torch
+    lin = lambda n: np.linspace(0.0, 1.0, n)
+    wl = make("poison2d", [lin(45), lin(37)], 2e-3, 40, [6, 6], [[A, A], [A, C]],
+              [[0.25, 0.75], [0.5, 0]], 11, drift=1.0, sigma=0.12)
+    ref = oracle_mod.Oracle(wl).algorithm1()
+    _, solve = fk
+    for _ in range(2):
+        junk = torch.full((96 << 20,), float("nan"), dtype=torch.float64, device="cuda")   # 768 MB
+        torch.cuda.synchronize()
+        del junk
+        torch.cuda.empty_cache()                            # hand the pages back to the driver
+        got = solve.evolve(wl)
+        assert np.isfinite(got).all()
         assert float(np.abs(got - ref).max()) <= TOL

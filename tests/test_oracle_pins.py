@@ -163,17 +163,48 @@ def test_constant_and_affine_fields_are_reproduced(oracle_mod, d):
     np.testing.assert_allclose(ones, 1.0, rtol=0, atol=1e-14)
 
 
-def test_bilinear_field_is_not_reproduced_in_2d(oracle_mod):
-    # Reading R4/A carries values + nodal gradient only: the mixed
-    # term x*y is NOT reproduced inside a cell, which tells reading A from a full tensor PCHIP.
-    wl = W.cellular_2d(n=(9, 9), N=2, Q=(1, 1))
+def _slope_bubble(h, t):
+    # sum of the two slope basis functions of Eq. 14 on a cell of width h at
+    # local coordinate t: h t (1-t)^2 + h t^2 (t-1) = h t (1-t) (1-2t)
+    return h * t * (1.0 - t) * (1.0 - 2.0 * t)
+
+
+def test_bilinear_field_exact_value_of_reading_A_in_2d(oracle_mod):
+    # Reading R4/A carries values + nodal gradient only.  For
+    # u = x*y the nodal slopes are exact (y along x-lines, x along y-lines) and the 1-D Hermite
+    # interpolant reproduces linear functions, so on any cell the interpolant of Eq. 13 is
+    #     x*y - s_x(t_x) * s_y(t_y),      s(t) = h t (1-t) (1-2t),
+    # the bilinear "bubble" a full tensor PCHIP would not have.  The value pins which corner each
+    # slope term of Eq. 13 is taken from: a slope read from the wrong corner changes the product.
+    wl = W.cellular_2d(n=(9, 9), N=2, Q=(1, 1))            # x in [0,2] h=1/4, y in [0,1] h=1/8
     X, Y = wl.mesh()
     o = oracle_mod.Oracle(wl)
     u = X * Y
-    z = np.array([[0.9, 0.43]])
-    val = o.interp(u, z)[0]
-    # A: corners (x0,y0)..; no mixed derivative => the error is the bilinear bubble
-    assert 1e-6 < abs(val - 0.9 * 0.43) < 1e-3
+    hx, hy = 0.25, 0.125
+    for zx, zy in [(0.9, 0.43), (1.3125, 0.07), (0.06, 0.99)]:
+        tx = (zx - math.floor(zx / hx) * hx) / hx
+        ty = (zy - math.floor(zy / hy) * hy) / hy
+        expect = zx * zy - _slope_bubble(hx, tx) * _slope_bubble(hy, ty)
+        val = o.interp(u, np.array([[zx, zy]]))[0]
+        assert abs(val - expect) < 2e-15, (zx, zy, val, expect)
+        assert abs(val - zx * zy) > 1e-7 or abs(_slope_bubble(hx, tx) * _slope_bubble(hy, ty)) < 1e-7
+
+
+def test_bilinear_fields_exact_value_of_reading_A_in_3d(oracle_mod):
+    # same in 3-D: u = x*y + y*z  ->  x*y + y*z - s_x s_y - s_y s_z (each product is bilinear in two
+    # coordinates and constant along the third, whose slope field is then 0)
+    wl = W.runaway_3d(n=(6, 9, 5), N=2, Q=(1, 1, 1))        # p in [0,50], xi in [-1,1], r in [0,1]
+    X, Y, Z = wl.mesh()
+    o = oracle_mod.Oracle(wl)
+    u = X * Y + Y * Z
+    h = [10.0, 0.25, 0.25]
+    lo = [0.0, -1.0, 0.0]
+    for z in [(13.7, -0.41, 0.33), (41.0, 0.62, 0.9), (2.5, -0.93, 0.05)]:
+        t = [((z[k] - lo[k]) - math.floor((z[k] - lo[k]) / h[k]) * h[k]) / h[k] for k in range(3)]
+        s = [_slope_bubble(h[k], t[k]) for k in range(3)]
+        expect = z[0] * z[1] + z[1] * z[2] - s[0] * s[1] - s[1] * s[2]
+        val = o.interp(u, np.array([z]))[0]
+        assert abs(val - expect) < 1e-14 * max(1.0, abs(expect)), (z, val, expect)
 
 
 def test_sigma_zero_is_a_pure_shift_and_zero_drift_is_identity(oracle_mod):
