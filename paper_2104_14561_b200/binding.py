@@ -19,8 +19,8 @@ FK_MEM_HOST, FK_MEM_DEVICE = 0, 1
 FK_ALL_STEPS = -1
 FK_MAX_Q = 32
 FK_FLAG_VALIDATE = 1
-FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_COUNT = 0, 1, 2, 3, 4
-KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused")
+FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_ROWBLOCK, FK_K_COUNT = 0, 1, 2, 3, 4, 5
+KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock")
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 

@@ -29,7 +29,9 @@ struct fk_ctx {
   double* d_coef = nullptr;            // [slots][2][d][J]: b then sigma per slot
   std::vector<int> slot_step;          // step held by each slot, -2 = empty
   bool autonomous = false;
-  double* d_P[2] = {nullptr, nullptr};
+  double* d_P[2] = {nullptr, nullptr};  // both point FK_GUARD_ROWS rows into their allocations
+  void* raw_P[2] = {nullptr, nullptr};
+  void* raw_dP = nullptr;
   int cur = 0;                         // buffer holding the current state
   double* d_dP = nullptr;
   // the operator of step nu is assembled on a side stream while the kernels of step nu+1 run:
@@ -142,9 +144,9 @@ void release(fk_ctx* c) {
   DeviceGuard guard(c->device);
   for (int k = 0; k < 3; ++k) { cudaFree(c->d_x[k]); cudaFree(c->d_invh[k]); }
   cudaFree(c->d_coef);
-  cudaFree(c->d_P[0]);
-  cudaFree(c->d_P[1]);
-  cudaFree(c->d_dP);
+  cudaFree(c->raw_P[0]);
+  cudaFree(c->raw_P[1]);
+  cudaFree(c->raw_dP);
   for (int i = 0; i < 2; ++i) {
     cudaFree(c->op[i].w);
     cudaFree(c->op[i].off);
@@ -288,9 +290,18 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     g.inv_h[k] = c->d_invh[k];
   }
   const size_t buf = sizeof(double) * (size_t)c->n_chunks * J * FK_CW;
-  FK_CREATE_CUDA(cudaMalloc(&c->d_P[0], buf));
-  FK_CREATE_CUDA(cudaMalloc(&c->d_P[1], buf));
-  FK_CREATE_CUDA(cudaMalloc(&c->d_dP, buf * p->d));
+  // P and dP carry FK_GUARD_ROWS zeroed 256-byte rows at both ends, and dP is cleared once: the
+  // row-blocked kernels read a few nodes past a line's ends with zero weights (fk_rowblock3d.cu),
+  // which must then be finite numbers
+  const size_t guard_bytes = sizeof(double) * FK_GUARD_ROWS * FK_CW;
+  for (int i = 0; i < 2; ++i) {
+    FK_CREATE_CUDA(cudaMalloc(&c->raw_P[i], buf + 2 * guard_bytes));
+    FK_CREATE_CUDA(cudaMemsetAsync(c->raw_P[i], 0, buf + 2 * guard_bytes, c->stream));
+    c->d_P[i] = reinterpret_cast<double*>(static_cast<char*>(c->raw_P[i]) + guard_bytes);
+  }
+  FK_CREATE_CUDA(cudaMalloc(&c->raw_dP, buf * p->d + 2 * guard_bytes));
+  FK_CREATE_CUDA(cudaMemsetAsync(c->raw_dP, 0, buf * p->d + 2 * guard_bytes, c->stream));
+  c->d_dP = reinterpret_cast<double*>(static_cast<char*>(c->raw_dP) + guard_bytes);
   FK_CREATE_CUDA(cudaMalloc(&c->d_coef, sizeof(double) * (size_t)slots * 2 * p->d * J));
   FK_CREATE_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
   FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_coef, cudaEventDisableTiming));
@@ -465,19 +476,25 @@ int evolve_step(fk_ctx* c, int n) {
       return fk_launch_fused2d(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, st); }));
   if (generic) {
     // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
-    long long sj0 = 0, sjn = c->g.J, aj0 = 0, ajn = c->g.J;
+    long long aj0 = 0, ajn = c->g.J;
+    int sl0 = 0, sln = (int)(c->g.J / c->g.n[c->g.d - 1]);
     if (fused) {
       const long long n1 = c->g.n[1];
       aj0 = (long long)(FK_FAR_BIG - far[1]) * n1;
       ajn = (long long)far[2] * n1 - aj0;
-      sj0 = (long long)(FK_FAR_BIG - far[3]) * n1;
-      sjn = (long long)far[4] * n1 - sj0;
+      sl0 = FK_FAR_BIG - far[3];
+      sln = far[4] - sl0;
     }
     FK_TRY(launch_on(c, st, FK_K_SLOPES, "fk_slopes", [&] {
-      return fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sj0, sjn, st); }));
-    FK_TRY(launch_on(c, st, FK_K_APPLY, "fk_apply", [&] {
-      return fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
-                             fused ? 1 : 0, aj0, ajn, st); }));
+      return fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sl0, sln, st); }));
+    if (c->g.d == 3)
+      FK_TRY(launch_on(c, st, FK_K_ROWBLOCK, "fk_rowblock3d", [&] {
+        return fk_launch_rowblock3d(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n,
+                                    c->N, st); }));
+    else
+      FK_TRY(launch_on(c, st, FK_K_APPLY, "fk_apply", [&] {
+        return fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
+                               fused ? 1 : 0, aj0, ajn, st); }));
   }
   FK_CUDA(c, cudaEventRecord(c->ev_free[ob], st));
   return FK_OK;

@@ -93,6 +93,82 @@ __device__ __forceinline__ double harmonic(double a, double b) {
   return p > 0.0 ? (p + p) * r : 0.0;
 }
 
+// One row of A_nu [P; dP] in factored form, contracted one dimension at a time (Eq. 13 with the
+// quadrature weights folded in):
+//   out = c_j + sum_{i0} [ alpha0 A'(i0) + beta0 B0'(i0) ]
+//   A'(i0)  = sum_{i1} [ alpha1 A(i0,i1) + beta1 B1(i0,i1) ],  B0'(i0) = sum_{i1} alpha1 B0(i0,i1)
+//   A(i0,i1)  = sum_{i2} [ alpha2 u + beta2 du2 ],  Bk(i0,i1) = sum_{i2} alpha2 du_k
+// w / off: the row's entries (alpha, beta) and element offsets; u, d0, d1, d2: the lane's column
+// of the chunk (base of the chunk + lane).
+template <int D>
+__device__ __forceinline__ double contract_row(const FkGrid& g, const double2* __restrict__ w,
+                                               const int* __restrict__ off, int4 cnt, double c,
+                                               const double* __restrict__ u,
+                                               const double* __restrict__ d0,
+                                               const double* __restrict__ d1,
+                                               const double* __restrict__ d2) {
+  double acc = c;
+  if (D == 1) {
+    double a0 = 0.0, a1 = 0.0;
+#pragma unroll 8
+    for (int e = 0; e < cnt.x; ++e) {
+      const double2 w0 = w[e];
+      const int o = off[e];
+      a0 = fma(w0.x, u[o], a0);
+      a1 = fma(w0.y, d0[o], a1);
+    }
+    acc += a0 + a1;
+  } else if (D == 2) {
+    const double2* __restrict__ w1p = w + g.qoff[1];
+    const int* __restrict__ o1p = off + g.qoff[1];
+    for (int e0 = 0; e0 < cnt.x; ++e0) {
+      const double2 w0 = w[e0];
+      const int o0 = off[e0];
+      double A = 0.0, A2 = 0.0, B0 = 0.0;
+#pragma unroll 4
+      for (int e1 = 0; e1 < cnt.y; ++e1) {
+        const double2 w1 = w1p[e1];
+        const int o = o0 + o1p[e1];
+        A = fma(w1.x, u[o], A);
+        A2 = fma(w1.y, d1[o], A2);
+        B0 = fma(w1.x, d0[o], B0);
+      }
+      acc = fma(w0.x, A + A2, acc);
+      acc = fma(w0.y, B0, acc);
+    }
+  } else {
+    const double2* __restrict__ w1p = w + g.qoff[1];
+    const int* __restrict__ o1p = off + g.qoff[1];
+    const double2* __restrict__ w2p = w + g.qoff[2];
+    const int* __restrict__ o2p = off + g.qoff[2];
+    for (int e0 = 0; e0 < cnt.x; ++e0) {
+      const double2 w0 = w[e0];
+      const int o0 = off[e0];
+      double Ap = 0.0, B0p = 0.0;
+      for (int e1 = 0; e1 < cnt.y; ++e1) {
+        const double2 w1 = w1p[e1];
+        const int o01 = o0 + o1p[e1];
+        double A = 0.0, A2 = 0.0, B0 = 0.0, B1 = 0.0;
+#pragma unroll 4
+        for (int e2 = 0; e2 < cnt.z; ++e2) {
+          const double2 w2 = w2p[e2];
+          const int o = o01 + o2p[e2];
+          A = fma(w2.x, u[o], A);
+          A2 = fma(w2.y, d2[o], A2);
+          B0 = fma(w2.x, d0[o], B0);
+          B1 = fma(w2.x, d1[o], B1);
+        }
+        Ap = fma(w1.x, A + A2, Ap);
+        Ap = fma(w1.y, B1, Ap);
+        B0p = fma(w1.x, B0, B0p);
+      }
+      acc = fma(w0.x, Ap, acc);
+      acc = fma(w0.y, B0p, acc);
+    }
+  }
+  return acc;
+}
+
 // ---- mbarrier / TMA bulk-copy primitives (sm_90+ PTX; SASS: SYNCS.*, UBLKCP)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);

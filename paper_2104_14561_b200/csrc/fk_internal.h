@@ -19,6 +19,7 @@
 
 #define FK_CW 32          // columns per chunk = lanes per warp
 #define FK_QMAX 32        // == FK_MAX_Q of include/fk.h
+#define FK_GUARD_ROWS 8   // zeroed node rows before and after the P and dP allocations
 
 struct FkGrid {
   int d;
@@ -95,12 +96,17 @@ cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold
                               int chunk0, int chunk1, int n, int N, int sm_count,
                               cudaStream_t s);
 cudaError_t fk_fused2d_setup(void);
-// slopes / apply on the nodes j0 .. j0+jn-1 only (jn = J: all nodes)
+// slopes of the lines line0 .. line0+nlines-1 (a line = one run of the fastest dimension; J / n[d-1]
+// lines in all); apply on the nodes j0 .. j0+jn-1 only (jn = J: all nodes)
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
-                             int chunk0, int chunk1, long long j0, long long jn, cudaStream_t s);
+                             int chunk0, int chunk1, int line0, int nlines, cudaStream_t s);
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
                             double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
                             int far_only, long long j0, long long jn, cudaStream_t s);
+// 3-D apply, four rows adjacent along dimension 2 per warp (fk_rowblock3d.cu); all rows
+cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* Pold,
+                                 const double* dP, double* Pnew, int n_chunks, int chunk0,
+                                 int chunk1, int n, int N, cudaStream_t s);
 cudaError_t fk_launch_gather_columns(const FkGrid& g, const double* P, int m0, int m1,
                                      double* out, cudaStream_t s);
 

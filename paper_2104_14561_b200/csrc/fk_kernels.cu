@@ -105,7 +105,7 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
     double2* wk = roww + g.qoff[k];
     int* ok = rowo + g.qoff[k];
 #define FK_EMIT(node, A, B)                                               \
-    do {                                                                  \
+    if ((A) != 0.0 || (B) != 0.0) {   /* exact zeros (a point on a node) are not entries */ \
       wk[count] = make_double2((A), (B));                                 \
       ok[count] = (int)((node) * unit);                                   \
       ++count;                                                            \
@@ -113,7 +113,7 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
         rec->w[k][(node) - rbase] = make_double2((A), (B));               \
         rmask |= 1 << ((node) - rbase);                                   \
       }                                                                   \
-    } while (0)
+    }
     for (int q = 0; q < g.Q[k]; ++q) {
       double z = fkd::push_point(centre, spread, g.gh_a[k][q]);
       const double w = g.gh_w[k][q];
@@ -214,40 +214,77 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
 }
 
 // ------------------------------------------------------------------------------------------
-// fk_slopes: block (32, 8): lane = column, threadIdx.y = node; grid.y = active chunks.
-// dP_k(j) from the grid line of axis k through j; end nodes use the first / last two
-// divided differences (R6).
+// fk_slopes<D>: dP_k(j) of Eq. 15 from the grid line of axis k through j, for every node of the
+// lines line0 .. line0+nlines-1 (a "line" = one run of the fastest dimension; its index runs over
+// the other dimensions) and every active chunk.  Block (32, 8): lane = column; a warp takes a
+// run of SR consecutive nodes of one line.  The fastest-dimension slopes come from the SR + 3
+// values around the run held in registers (one load per node); each other dimension needs the
+// two neighbours across lines.  End nodes use the first / last two divided differences (R6,
+// PAPER.md:160): with la = clamp(i-1, 0, n-3) the three nodes la, la+1, la+2 give both cases.
 // ------------------------------------------------------------------------------------------
-__global__ void fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP,
-                          int n_chunks, int chunk0, long long j0, long long jn) {
-  long long j = (long long)blockIdx.x * blockDim.y + threadIdx.y;
-  if (j >= jn) return;
-  j += j0;
+constexpr int SR = 8;
+
+template <int D>
+__global__ void __launch_bounds__(256)
+fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP, int n_chunks,
+          int chunk0, int line0, int nlines) {
+  const int nl = g.n[D - 1];
+  const int segs = (nl + SR - 1) / SR;
+  const int rid = blockIdx.x * 8 + threadIdx.y;
+  if (rid >= nlines * segs) return;
+  const int line = line0 + rid / segs;
+  const int i0 = (rid - (rid / segs) * segs) * SR;
   const int c = chunk0 + blockIdx.y;
-  int idx[3];
-  unravel(g, j, idx);
   const size_t chunk_elems = (size_t)g.J * FK_CW;
-  const double* __restrict__ u = P + (size_t)c * chunk_elems + (size_t)j * FK_CW + threadIdx.x;
-  const double u0 = u[0];
-  for (int k = 0; k < g.d; ++k) {
-    const long long s = g.stride[k] * FK_CW;
-    const int i = idx[k], n = g.n[k];
-    const double* __restrict__ ih = g.inv_h[k];
-    double da, db;
-    if (i == 0) {
-      const double u1 = u[s], u2 = u[2 * s];
-      da = (u1 - u0) * ih[0];
-      db = (u2 - u1) * ih[1];
-    } else if (i == n - 1) {
-      const double u1 = u[-s], u2 = u[-2 * s];
-      da = (u0 - u1) * ih[n - 2];
-      db = (u1 - u2) * ih[n - 3];
-    } else {
-      da = (u0 - u[-s]) * ih[i - 1];
-      db = (u[s] - u0) * ih[i];
+  const int node0 = line * nl;                                   // node (line, 0)
+  const double* __restrict__ u = P + (size_t)c * chunk_elems + (size_t)node0 * FK_CW + threadIdx.x;
+  double* __restrict__ o = dP + (size_t)c * chunk_elems + (size_t)node0 * FK_CW + threadIdx.x;
+  const size_t field = (size_t)n_chunks * chunk_elems;
+
+  // values of the line at nodes i0-2 .. i0+SR (clamped; clamped duplicates are never selected)
+  double v[SR + 3];
+#pragma unroll
+  for (int k = 0; k < SR + 3; ++k) v[k] = u[min(max(i0 - 2 + k, 0), nl - 1) * FK_CW];
+  {
+    const double* __restrict__ ih = g.inv_h[D - 1];
+    double dl[SR + 2];                                           // dl[k]: cell right of node i0-2+k
+#pragma unroll
+    for (int k = 0; k < SR + 2; ++k) dl[k] = (v[k + 1] - v[k]) * ih[min(max(i0 - 2 + k, 0), nl - 2)];
+    double* __restrict__ ok = o + (size_t)(D - 1) * field;
+#pragma unroll
+    for (int k = 0; k < SR; ++k) {
+      const int i = i0 + k;
+      if (i < nl) {
+        const double a = i == 0 ? dl[2] : (i == nl - 1 ? dl[k] : dl[k + 1]);
+        const double b = i == 0 ? dl[3] : (i == nl - 1 ? dl[k + 1] : dl[k + 2]);
+        ok[i * FK_CW] = harmonic(a, b);
+      }
     }
-    dP[((size_t)k * n_chunks + c) * chunk_elems + (size_t)j * FK_CW + threadIdx.x] =
-        harmonic(da, db);
+  }
+  if (D >= 2) {
+    int idx[2];
+    idx[0] = D == 3 ? line / g.n[1] : line;
+    idx[1] = D == 3 ? line - idx[0] * g.n[1] : 0;
+#pragma unroll
+    for (int k = 0; k < D - 1; ++k) {
+      const int nk = g.n[k], ik = idx[k];
+      const int la = min(max(ik - 1, 0), nk - 3);
+      const int s = (int)g.stride[k] * FK_CW;
+      const int oa = (la - ik) * s, ob = oa + s, oc = ob + s;    // one of them may be 0 (the node)
+      const double iha = g.inv_h[k][la], ihb = g.inv_h[k][la + 1];
+      double* __restrict__ ok = o + (size_t)k * field;
+#pragma unroll
+      for (int q = 0; q < SR; ++q) {
+        const int i = i0 + q;
+        if (i < nl) {
+          const double* __restrict__ un = u + i * FK_CW;
+          const double va = oa == 0 ? v[q + 2] : un[oa];
+          const double vb = ob == 0 ? v[q + 2] : un[ob];
+          const double vc = oc == 0 ? v[q + 2] : un[oc];
+          ok[i * FK_CW] = harmonic((vb - va) * iha, (vc - vb) * ihb);
+        }
+      }
+    }
   }
 }
 
@@ -278,65 +315,7 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   const int* __restrict__ off = op.off + (size_t)j * g.RS;
   const int4 cnt = *reinterpret_cast<const int4*>(op.cnt + j * 4);
   if (far_only && (cnt.w & (FK_ROW_NEAR | FK_ROW_DIRICHLET))) return;   // done by fk_fused2d
-  double acc = op.c[j];
-  if (D == 1) {
-    double a0 = 0.0, a1 = 0.0;
-#pragma unroll 8
-    for (int e = 0; e < cnt.x; ++e) {
-      const double2 w0 = w[e];
-      const int o = off[e];
-      a0 = fma(w0.x, u[o], a0);
-      a1 = fma(w0.y, d0[o], a1);
-    }
-    acc += a0 + a1;
-  } else if (D == 2) {
-    const double2* __restrict__ w1p = w + g.qoff[1];
-    const int* __restrict__ o1p = off + g.qoff[1];
-    for (int e0 = 0; e0 < cnt.x; ++e0) {
-      const double2 w0 = w[e0];
-      const int o0 = off[e0];
-      double A = 0.0, A2 = 0.0, B0 = 0.0;
-#pragma unroll 4
-      for (int e1 = 0; e1 < cnt.y; ++e1) {
-        const double2 w1 = w1p[e1];
-        const int o = o0 + o1p[e1];
-        A = fma(w1.x, u[o], A);
-        A2 = fma(w1.y, d1[o], A2);
-        B0 = fma(w1.x, d0[o], B0);
-      }
-      acc = fma(w0.x, A + A2, acc);
-      acc = fma(w0.y, B0, acc);
-    }
-  } else {
-    const double2* __restrict__ w1p = w + g.qoff[1];
-    const int* __restrict__ o1p = off + g.qoff[1];
-    const double2* __restrict__ w2p = w + g.qoff[2];
-    const int* __restrict__ o2p = off + g.qoff[2];
-    for (int e0 = 0; e0 < cnt.x; ++e0) {
-      const double2 w0 = w[e0];
-      const int o0 = off[e0];
-      double Ap = 0.0, B0p = 0.0;
-      for (int e1 = 0; e1 < cnt.y; ++e1) {
-        const double2 w1 = w1p[e1];
-        const int o01 = o0 + o1p[e1];
-        double A = 0.0, A2 = 0.0, B0 = 0.0, B1 = 0.0;
-#pragma unroll 4
-        for (int e2 = 0; e2 < cnt.z; ++e2) {
-          const double2 w2 = w2p[e2];
-          const int o = o01 + o2p[e2];
-          A = fma(w2.x, u[o], A);
-          A2 = fma(w2.y, d2[o], A2);
-          B0 = fma(w2.x, d0[o], B0);
-          B1 = fma(w2.x, d1[o], B1);
-        }
-        Ap = fma(w1.x, A + A2, Ap);
-        Ap = fma(w1.y, B1, Ap);
-        B0p = fma(w1.x, B0, B0p);
-      }
-      acc = fma(w0.x, Ap, acc);
-      acc = fma(w0.y, B0p, acc);
-    }
-  }
+  const double acc = fkd::contract_row<D>(g, w, off, cnt, op.c[j], u, d0, d1, d2);
   if (m >= n && m <= N) Pnew[(size_t)c * chunk_elems + (size_t)j * FK_CW + threadIdx.x] = acc;
 }
 
@@ -390,9 +369,12 @@ cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, i
 }
 
 cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n_chunks,
-                             int chunk0, int chunk1, long long j0, long long jn, cudaStream_t s) {
-  dim3 block(FK_CW, 8), grid((unsigned)((jn + 7) / 8), (unsigned)(chunk1 - chunk0));
-  fk_slopes<<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0, j0, jn);
+                             int chunk0, int chunk1, int line0, int nlines, cudaStream_t s) {
+  const int segs = (g.n[g.d - 1] + SR - 1) / SR;
+  dim3 block(FK_CW, 8), grid((unsigned)(((long long)nlines * segs + 7) / 8), (unsigned)(chunk1 - chunk0));
+  if (g.d == 1) fk_slopes<1><<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0, line0, nlines);
+  else if (g.d == 2) fk_slopes<2><<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0, line0, nlines);
+  else fk_slopes<3><<<grid, block, 0, s>>>(g, P, dP, n_chunks, chunk0, line0, nlines);
   return cudaGetLastError();
 }
 

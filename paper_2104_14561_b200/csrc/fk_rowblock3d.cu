@@ -1,0 +1,249 @@
+// fk_rowblock3d.cu -- the 3-D apply kernel: P(:, n:N) <- A_nu [P; dP](:, n:N) with
+// the rows of A_nu taken FOUR AT A TIME.
+//
+// Lane = output-time column of a 32-column chunk, as everywhere in this library; a warp owns a
+// group of RB = 4 rows that are adjacent along the fastest dimension (dimension 2).  In the
+// factored row (fk_internal.h) the weights of dimension 0 and 1 multiply whole dimension-2 runs,
+//     out_r = c_r + sum_{e0, e1} [ a0 a1 (A_r + A2_r) + a0 b1 B1_r + b0 a1 B0_r ],
+//     A_r = sum_t alpha2_r(t) u(e0, e1, i2_r + t), ...  (fkd::contract_row),
+// so when the four rows put their dimension-0 and dimension-1 entries on the SAME nodes (drift and
+// diffusion vary slowly along dimension 2: the usual case) the four inner sums read the same
+// run of RB + 2H nodes: every u / dP value is loaded once per group and feeds up to RB rows,
+// with the dimension-2 weights in registers at static indices (slot t of row r is union node
+// q = r + t, as in the fused 2-D kernel).  The kernel body is instantiated for the slot ranges
+// that occur (own node only -- where the dimension-2 motion vanishes a group reads 4 nodes --,
+// +-1, ..., all 2H+1), chosen per group by a warp-uniform test.
+// Groups whose rows disagree (a quadrature point of one row falls into the next cell), reach
+// beyond H nodes along dimension 2, or have more than EMAX entries in dimension 0 or 1, take the
+// row-at-a-time path (fkd::contract_row) inside the same kernel.
+//
+// u and dP come from global memory through L1: a block is 4 warps = the same dimension-2 group of
+// 4 consecutive dimension-1 lines, whose dimension-0 / dimension-1 nodes largely coincide.
+#include "fk_device.cuh"
+
+namespace {
+
+constexpr int RB = 4;                      // rows per warp
+constexpr int H2 = FK_H;                   // dimension-2 halo of the blocked path
+constexpr int NS = 2 * H2 + 1;             // slots per row along dimension 2
+constexpr int NU = RB + NS - 1;            // union nodes of a group
+constexpr int EMAX = 16;                   // entries per row in dimension 0 / 1 (blocked path)
+constexpr int WARPS = 4;
+
+struct GroupStage {                        // per warp, shared memory
+  double2 w0[RB][EMAX];
+  double2 w1[RB][EMAX];
+  double2 w2[RB][NS];
+  int off0[EMAX], off1[EMAX];
+  double c[RB];
+};
+
+// The contraction of a group whose rows use only the dimension-2 slots TLO..THI: union nodes
+// q = TLO .. RB-1+THI of the run starting at ub / d0b / ... (node i2b - H2).  Every load has a
+// compile-time offset and no predicate; a union node outside the line (first / last group) is a
+// node of the neighbouring line, chunk or guard row -- finite values that only ever meet zero
+// weights (fk_api.cu allocates P and dP with guard rows at both ends).
+template <int TLO, int THI>
+__device__ __forceinline__ void contract_group(const GroupStage& st, int4 cref,
+                                               const double* __restrict__ ub,
+                                               const double* __restrict__ d0b,
+                                               const double* __restrict__ d1b,
+                                               const double* __restrict__ d2b, double acc[RB]) {
+  constexpr int Q0 = TLO, Q1 = RB - 1 + THI;             // first / last union node
+  double2 w2[RB][THI - TLO + 1];
+#pragma unroll
+  for (int r = 0; r < RB; ++r) {
+    acc[r] = st.c[r];
+#pragma unroll
+    for (int t = TLO; t <= THI; ++t) w2[r][t - TLO] = st.w2[r][t];
+  }
+  for (int e0 = 0; e0 < cref.x; ++e0) {
+    const int o0 = st.off0[e0];
+    double Ap[RB], B0p[RB];
+#pragma unroll
+    for (int r = 0; r < RB; ++r) Ap[r] = B0p[r] = 0.0;
+    for (int e1 = 0; e1 < cref.y; ++e1) {
+      const int o = o0 + st.off1[e1];
+      const double* __restrict__ pu = ub + o;
+      const double* __restrict__ p0 = d0b + o;
+      const double* __restrict__ p1 = d1b + o;
+      const double* __restrict__ p2 = d2b + o;
+      double U[Q1 - Q0 + 1], D0[Q1 - Q0 + 1], D1[Q1 - Q0 + 1], D2[Q1 - Q0 + 1];
+#pragma unroll
+      for (int q = Q0; q <= Q1; ++q) {                   // all loads of the pair first
+        U[q - Q0] = pu[q * FK_CW];
+        D0[q - Q0] = p0[q * FK_CW];
+        D1[q - Q0] = p1[q * FK_CW];
+        D2[q - Q0] = p2[q * FK_CW];
+      }
+      double A[RB], B0[RB], B1[RB];
+#pragma unroll
+      for (int r = 0; r < RB; ++r) A[r] = B0[r] = B1[r] = 0.0;
+#pragma unroll
+      for (int q = Q0; q <= Q1; ++q) {
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+          const int t = q - r;
+          if (t >= TLO && t <= THI) {
+            A[r] = fma(w2[r][t - TLO].x, U[q - Q0], A[r]);
+            A[r] = fma(w2[r][t - TLO].y, D2[q - Q0], A[r]);
+            B0[r] = fma(w2[r][t - TLO].x, D0[q - Q0], B0[r]);
+            B1[r] = fma(w2[r][t - TLO].x, D1[q - Q0], B1[r]);
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < RB; ++r) {
+        const double2 w1 = st.w1[r][e1];
+        Ap[r] = fma(w1.x, A[r], Ap[r]);
+        Ap[r] = fma(w1.y, B1[r], Ap[r]);
+        B0p[r] = fma(w1.x, B0[r], B0p[r]);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      const double2 w0 = st.w0[r][e0];
+      acc[r] = fma(w0.x, Ap[r], acc[r]);
+      acc[r] = fma(w0.y, B0p[r], acc[r]);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(WARPS * 32, 3)
+fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
+              const double* __restrict__ dP, double* __restrict__ Pnew, int n_chunks, int chunk0,
+              int n, int N, int G2, int NT1) {
+  __shared__ GroupStage stage_all[WARPS];
+  GroupStage& st = stage_all[threadIdx.y];
+  const int lane = threadIdx.x;
+  const int n1 = g.n[1], n2 = g.n[2];
+  const int g2 = blockIdx.x % G2;
+  const int t01 = blockIdx.x / G2;
+  const int i1 = (t01 % NT1) * WARPS + threadIdx.y;
+  const int i0 = t01 / NT1;
+  if (i1 >= n1) return;
+  const int i2b = g2 * RB;
+  const int rows = min(RB, n2 - i2b);
+  const int jb = (i0 * n1 + i1) * n2 + i2b;
+  const int chunk = chunk0 + blockIdx.y;
+  const int m = chunk * FK_CW + lane;
+  const bool active = m >= n && m <= N;
+  const size_t chunk_elems = (size_t)g.J * FK_CW;
+  const double* __restrict__ u = Pold + (size_t)chunk * chunk_elems + lane;
+  const double* __restrict__ d0 = dP + (size_t)chunk * chunk_elems + lane;
+  const double* __restrict__ d1 = d0 + (size_t)n_chunks * chunk_elems;
+  const double* __restrict__ d2 = d1 + (size_t)n_chunks * chunk_elems;
+  double* __restrict__ out = Pnew + (size_t)chunk * chunk_elems + (size_t)jb * FK_CW + lane;
+
+  // ---- stage the group's rows; decide whether they can be contracted together
+  int4 cnt[RB];
+  int4 cref = make_int4(0, 0, 0, 0);
+  int ref = -1;                                         // first row that is not a Dirichlet row
+#pragma unroll
+  for (int r = 0; r < RB; ++r) {
+    cnt[r] = r < rows ? *reinterpret_cast<const int4*>(op.cnt + (size_t)(jb + r) * 4)
+                      : make_int4(0, 0, 0, FK_ROW_DIRICHLET);
+    if (ref < 0 && !(cnt[r].w & FK_ROW_DIRICHLET)) { ref = r; cref = cnt[r]; }
+  }
+  if (ref < 0) {                                        // only Dirichlet rows: the constants
+    for (int r = 0; r < rows; ++r)
+      if (active) out[r * FK_CW] = op.c[jb + r];
+    return;
+  }
+  // every load of the stage is issued before anything is compared (one round of latency)
+  bool ok = cref.x <= EMAX && cref.y <= EMAX;
+  {
+    const int dim = lane >> 4, e = lane & (EMAX - 1);   // lanes 0..15: dimension 0, 16..31: 1
+    const int ne_ref = dim ? cref.y : cref.x;
+    const bool mine = ok && e < ne_ref;
+    const int q = g.qoff[dim] + e;
+    const int q2 = g.qoff[2] + lane;
+    int off01[RB], off2[RB];
+    double2 w01[RB], w2[RB];
+    double cr = 0.0;
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      const bool dir = (cnt[r].w & FK_ROW_DIRICHLET) != 0;
+      const size_t row = (size_t)(jb + r) * g.RS;
+      off01[r] = -1;
+      off2[r] = 0;
+      w01[r] = w2[r] = make_double2(0.0, 0.0);
+      if (!dir && mine) { off01[r] = op.off[row + q]; w01[r] = op.w[row + q]; }
+      if (!dir && lane < cnt[r].z && lane < NS) { off2[r] = op.off[row + q2]; w2[r] = op.w[row + q2]; }
+      if (lane == r && r < rows) cr = op.c[jb + r];
+    }
+    int oref = -1;
+#pragma unroll
+    for (int r = 0; r < RB; ++r) if (r == ref) oref = off01[r];
+    if (dim) st.off1[e] = oref; else st.off0[e] = oref;
+    if (lane < RB * NS) st.w2[lane / NS][lane % NS] = make_double2(0.0, 0.0);
+    if (lane < RB) st.c[lane] = cr;
+    __syncwarp();
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      const bool dir = (cnt[r].w & FK_ROW_DIRICHLET) != 0;
+      if (dim) st.w1[r][e] = w01[r]; else st.w0[r][e] = w01[r];
+      if (dir) continue;
+      ok = ok && cnt[r].x == cref.x && cnt[r].y == cref.y && cnt[r].z <= NS && off01[r] == oref;
+      if (lane < cnt[r].z && lane < NS) {
+        // dimension 2: entries -> slots around the row's own node (its stride is 1 node)
+        const int t = off2[r] / FK_CW - (i2b + r) + H2;
+        if (t >= 0 && t < NS) st.w2[r][t] = w2[r];
+        else ok = false;
+      }
+    }
+  }
+  ok = __all_sync(0xffffffffu, ok);
+  __syncwarp();
+
+  if (!ok) {
+    // ---- row-at-a-time path
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      if (r < rows) {
+        const size_t j = (size_t)(jb + r);
+        const double acc = fkd::contract_row<3>(g, op.w + j * g.RS, op.off + j * g.RS, cnt[r],
+                                                op.c[j], u, d0, d1, d2);
+        if (active) out[r * FK_CW] = acc;
+      }
+    }
+    return;
+  }
+
+  // ---- blocked path: which dimension-2 slots carry a weight in any row decides the variant
+  unsigned tmask = 0;
+#pragma unroll
+  for (int r = 0; r < RB; ++r)
+#pragma unroll
+    for (int t = 0; t < NS; ++t) {
+      const double2 w = st.w2[r][t];
+      if (w.x != 0.0 || w.y != 0.0) tmask |= 1u << t;
+    }
+  tmask = __reduce_or_sync(0xffffffffu, tmask);          // uniform
+  double acc[RB];
+  const int base2 = (i2b - H2) * FK_CW;                  // union node 0
+  const double* __restrict__ ub = u + base2;
+  const double* __restrict__ d0b = d0 + base2;
+  const double* __restrict__ d1b = d1 + base2;
+  const double* __restrict__ d2b = d2 + base2;
+  if ((tmask & ~0x04u) == 0) contract_group<2, 2>(st, cref, ub, d0b, d1b, d2b, acc);
+  else if ((tmask & ~0x06u) == 0) contract_group<1, 2>(st, cref, ub, d0b, d1b, d2b, acc);
+  else if ((tmask & ~0x0cu) == 0) contract_group<2, 3>(st, cref, ub, d0b, d1b, d2b, acc);
+  else if ((tmask & ~0x0eu) == 0) contract_group<1, 3>(st, cref, ub, d0b, d1b, d2b, acc);
+  else contract_group<0, 4>(st, cref, ub, d0b, d1b, d2b, acc);
+#pragma unroll
+  for (int r = 0; r < RB; ++r)
+    if (r < rows && active) out[r * FK_CW] = acc[r];
+}
+
+}  // namespace
+
+cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* Pold,
+                                 const double* dP, double* Pnew, int n_chunks, int chunk0,
+                                 int chunk1, int n, int N, cudaStream_t s) {
+  const int G2 = (g.n[2] + RB - 1) / RB;
+  const int NT1 = (g.n[1] + WARPS - 1) / WARPS;
+  dim3 block(FK_CW, WARPS), grid((unsigned)((long long)g.n[0] * NT1 * G2), (unsigned)(chunk1 - chunk0));
+  fk_rowblock3d<<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, G2, NT1);
+  return cudaGetLastError();
+}
