@@ -28,7 +28,10 @@ constexpr int H2 = FK_H;                   // dimension-2 halo of the blocked pa
 constexpr int NS = 2 * H2 + 1;             // slots per row along dimension 2
 constexpr int NU = RB + NS - 1;            // union nodes of a group
 constexpr int EMAX = 16;                   // entries per row in dimension 0 / 1 (blocked path)
-constexpr int WARPS = 4;
+constexpr int WARPS = 4;                   // a block = the same dimension-2 group of 4 dimension-1 lines
+constexpr int MINB = 3;                    // blocks per SM the register budget is set for
+constexpr int CPB = 2;                     // chunks served by one staging of a group's rows
+constexpr int L2PF = 3;                    // planes ahead whose rows a group pulls into L2
 
 struct GroupStage {                        // per warp, shared memory
   double2 w0[RB][EMAX];
@@ -43,76 +46,92 @@ struct GroupStage {                        // per warp, shared memory
 // compile-time offset and no predicate; a union node outside the line (first / last group) is a
 // node of the neighbouring line, chunk or guard row -- finite values that only ever meet zero
 // weights (fk_api.cu allocates P and dP with guard rows at both ends).
+// All loads of a pair (4 fields x up to RB + 2H nodes) are issued before its arithmetic.
+template <int NQ>
+struct PairVals {
+  double U[NQ], D0[NQ], D1[NQ], D2[NQ];
+};
+
 template <int TLO, int THI>
 __device__ __forceinline__ void contract_group(const GroupStage& st, int4 cref,
                                                const double* __restrict__ ub,
                                                const double* __restrict__ d0b,
                                                const double* __restrict__ d1b,
                                                const double* __restrict__ d2b, double acc[RB]) {
-  constexpr int Q0 = TLO, Q1 = RB - 1 + THI;             // first / last union node
+  constexpr int Q0 = TLO, Q1 = RB - 1 + THI, NQ = Q1 - Q0 + 1;   // union nodes Q0..Q1
   double2 w2[RB][THI - TLO + 1];
+  double Ap[RB], B0p[RB];
 #pragma unroll
   for (int r = 0; r < RB; ++r) {
     acc[r] = st.c[r];
+    Ap[r] = B0p[r] = 0.0;
 #pragma unroll
     for (int t = TLO; t <= THI; ++t) w2[r][t - TLO] = st.w2[r][t];
   }
-  for (int e0 = 0; e0 < cref.x; ++e0) {
-    const int o0 = st.off0[e0];
-    double Ap[RB], B0p[RB];
+  const int n0e = cref.x, n1e = cref.y;
+  auto load = [&](PairVals<NQ>& v, int e0, int e1) {
+    const int o = st.off0[e0] + st.off1[e1] + Q0 * FK_CW;
+    const double* __restrict__ pu = ub + o;
+    const double* __restrict__ p0 = d0b + o;
+    const double* __restrict__ p1 = d1b + o;
+    const double* __restrict__ p2 = d2b + o;
 #pragma unroll
-    for (int r = 0; r < RB; ++r) Ap[r] = B0p[r] = 0.0;
-    for (int e1 = 0; e1 < cref.y; ++e1) {
-      const int o = o0 + st.off1[e1];
-      const double* __restrict__ pu = ub + o;
-      const double* __restrict__ p0 = d0b + o;
-      const double* __restrict__ p1 = d1b + o;
-      const double* __restrict__ p2 = d2b + o;
-      double U[Q1 - Q0 + 1], D0[Q1 - Q0 + 1], D1[Q1 - Q0 + 1], D2[Q1 - Q0 + 1];
+    for (int q = 0; q < NQ; ++q) {
+      v.U[q] = pu[q * FK_CW];
+      v.D0[q] = p0[q * FK_CW];
+      v.D1[q] = p1[q * FK_CW];
+      v.D2[q] = p2[q * FK_CW];
+    }
+  };
+  auto compute = [&](const PairVals<NQ>& v, int e0, int e1) {
+    double A[RB], B0[RB], B1[RB];
 #pragma unroll
-      for (int q = Q0; q <= Q1; ++q) {                   // all loads of the pair first
-        U[q - Q0] = pu[q * FK_CW];
-        D0[q - Q0] = p0[q * FK_CW];
-        D1[q - Q0] = p1[q * FK_CW];
-        D2[q - Q0] = p2[q * FK_CW];
-      }
-      double A[RB], B0[RB], B1[RB];
+    for (int r = 0; r < RB; ++r) A[r] = B0[r] = B1[r] = 0.0;
 #pragma unroll
-      for (int r = 0; r < RB; ++r) A[r] = B0[r] = B1[r] = 0.0;
-#pragma unroll
-      for (int q = Q0; q <= Q1; ++q) {
-#pragma unroll
-        for (int r = 0; r < RB; ++r) {
-          const int t = q - r;
-          if (t >= TLO && t <= THI) {
-            A[r] = fma(w2[r][t - TLO].x, U[q - Q0], A[r]);
-            A[r] = fma(w2[r][t - TLO].y, D2[q - Q0], A[r]);
-            B0[r] = fma(w2[r][t - TLO].x, D0[q - Q0], B0[r]);
-            B1[r] = fma(w2[r][t - TLO].x, D1[q - Q0], B1[r]);
-          }
-        }
-      }
+    for (int q = Q0; q <= Q1; ++q) {
 #pragma unroll
       for (int r = 0; r < RB; ++r) {
-        const double2 w1 = st.w1[r][e1];
-        Ap[r] = fma(w1.x, A[r], Ap[r]);
-        Ap[r] = fma(w1.y, B1[r], Ap[r]);
-        B0p[r] = fma(w1.x, B0[r], B0p[r]);
+        const int t = q - r;
+        if (t >= TLO && t <= THI) {
+          const double2 w = w2[r][t - TLO];
+          A[r] = fma(w.x, v.U[q - Q0], A[r]);
+          A[r] = fma(w.y, v.D2[q - Q0], A[r]);
+          B0[r] = fma(w.x, v.D0[q - Q0], B0[r]);
+          B1[r] = fma(w.x, v.D1[q - Q0], B1[r]);
+        }
       }
     }
 #pragma unroll
     for (int r = 0; r < RB; ++r) {
-      const double2 w0 = st.w0[r][e0];
-      acc[r] = fma(w0.x, Ap[r], acc[r]);
-      acc[r] = fma(w0.y, B0p[r], acc[r]);
+      const double2 w1 = st.w1[r][e1];
+      Ap[r] = fma(w1.x, A[r], Ap[r]);
+      Ap[r] = fma(w1.y, B1[r], Ap[r]);
+      B0p[r] = fma(w1.x, B0[r], B0p[r]);
     }
-  }
+    if (e1 == n1e - 1) {                                 // last pair of this e0: fold it in
+#pragma unroll
+      for (int r = 0; r < RB; ++r) {
+        const double2 w0 = st.w0[r][e0];
+        acc[r] = fma(w0.x, Ap[r], acc[r]);
+        acc[r] = fma(w0.y, B0p[r], acc[r]);
+        Ap[r] = B0p[r] = 0.0;
+      }
+    }
+  };
+  const int pairs = n0e * n1e;
+  if (pairs == 0) return;
+  PairVals<NQ> v;
+  for (int e0 = 0; e0 < n0e; ++e0)
+    for (int e1 = 0; e1 < n1e; ++e1) {
+      load(v, e0, e1);
+      compute(v, e0, e1);
+    }
 }
 
-__global__ void __launch_bounds__(WARPS * 32, 3)
+__global__ void __launch_bounds__(WARPS * 32, MINB)
 fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
               const double* __restrict__ dP, double* __restrict__ Pnew, int n_chunks, int chunk0,
-              int n, int N, int G2, int NT1) {
+              int chunk1, int n, int N, int G2, int NT1) {
   __shared__ GroupStage stage_all[WARPS];
   GroupStage& st = stage_all[threadIdx.y];
   const int lane = threadIdx.x;
@@ -125,15 +144,10 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   const int i2b = g2 * RB;
   const int rows = min(RB, n2 - i2b);
   const int jb = (i0 * n1 + i1) * n2 + i2b;
-  const int chunk = chunk0 + blockIdx.y;
-  const int m = chunk * FK_CW + lane;
-  const bool active = m >= n && m <= N;
+  // the staged rows serve CPB consecutive chunks: blockIdx.y counts chunk groups
+  const int cfirst = chunk0 + blockIdx.y * CPB, clast = min(chunk1, cfirst + CPB);
   const size_t chunk_elems = (size_t)g.J * FK_CW;
-  const double* __restrict__ u = Pold + (size_t)chunk * chunk_elems + lane;
-  const double* __restrict__ d0 = dP + (size_t)chunk * chunk_elems + lane;
-  const double* __restrict__ d1 = d0 + (size_t)n_chunks * chunk_elems;
-  const double* __restrict__ d2 = d1 + (size_t)n_chunks * chunk_elems;
-  double* __restrict__ out = Pnew + (size_t)chunk * chunk_elems + (size_t)jb * FK_CW + lane;
+  const size_t field = (size_t)n_chunks * chunk_elems;
 
   // ---- stage the group's rows; decide whether they can be contracted together
   int4 cnt[RB];
@@ -146,8 +160,12 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     if (ref < 0 && !(cnt[r].w & FK_ROW_DIRICHLET)) { ref = r; cref = cnt[r]; }
   }
   if (ref < 0) {                                        // only Dirichlet rows: the constants
-    for (int r = 0; r < rows; ++r)
-      if (active) out[r * FK_CW] = op.c[jb + r];
+    for (int chunk = cfirst; chunk < clast; ++chunk) {
+      const int m = chunk * FK_CW + lane;
+      double* __restrict__ out = Pnew + (size_t)chunk * chunk_elems + (size_t)jb * FK_CW + lane;
+      for (int r = 0; r < rows; ++r)
+        if (m >= n && m <= N) out[r * FK_CW] = op.c[jb + r];
+    }
     return;
   }
   // every load of the stage is issued before anything is compared (one round of latency)
@@ -196,21 +214,7 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   ok = __all_sync(0xffffffffu, ok);
   __syncwarp();
 
-  if (!ok) {
-    // ---- row-at-a-time path
-#pragma unroll
-    for (int r = 0; r < RB; ++r) {
-      if (r < rows) {
-        const size_t j = (size_t)(jb + r);
-        const double acc = fkd::contract_row<3>(g, op.w + j * g.RS, op.off + j * g.RS, cnt[r],
-                                                op.c[j], u, d0, d1, d2);
-        if (active) out[r * FK_CW] = acc;
-      }
-    }
-    return;
-  }
-
-  // ---- blocked path: which dimension-2 slots carry a weight in any row decides the variant
+  // ---- which dimension-2 slots carry a weight in any row decides the variant of the blocked path
   unsigned tmask = 0;
 #pragma unroll
   for (int r = 0; r < RB; ++r)
@@ -220,20 +224,60 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
       if (w.x != 0.0 || w.y != 0.0) tmask |= 1u << t;
     }
   tmask = __reduce_or_sync(0xffffffffu, tmask);          // uniform
-  double acc[RB];
   const int base2 = (i2b - H2) * FK_CW;                  // union node 0
-  const double* __restrict__ ub = u + base2;
-  const double* __restrict__ d0b = d0 + base2;
-  const double* __restrict__ d1b = d1 + base2;
-  const double* __restrict__ d2b = d2 + base2;
-  if ((tmask & ~0x04u) == 0) contract_group<2, 2>(st, cref, ub, d0b, d1b, d2b, acc);
-  else if ((tmask & ~0x06u) == 0) contract_group<1, 2>(st, cref, ub, d0b, d1b, d2b, acc);
-  else if ((tmask & ~0x0cu) == 0) contract_group<2, 3>(st, cref, ub, d0b, d1b, d2b, acc);
-  else if ((tmask & ~0x0eu) == 0) contract_group<1, 3>(st, cref, ub, d0b, d1b, d2b, acc);
-  else contract_group<0, 4>(st, cref, ub, d0b, d1b, d2b, acc);
+
+  // pull this group's own rows of the plane L2PF steps ahead into L2 (one bulk prefetch
+  // per field): the blocks that will read them find them there instead of in DRAM
+  if (lane < 4 && i0 + L2PF < g.n[0]) {
+    const size_t ahead = (size_t)(jb + L2PF * n1 * n2) * FK_CW;
+    for (int chunk = cfirst; chunk < clast; ++chunk) {
+      const double* src = (lane == 0 ? Pold : dP + (size_t)(lane - 1) * field) + (size_t)chunk * chunk_elems + ahead;
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(rows * FK_CW * 8) : "memory");
+    }
+  }
+  if (lane >= 4 && lane < 7 && blockIdx.y == 0 && i0 + L2PF < g.n[0]) {   // and the operator rows
+    const size_t ja = (size_t)jb + (size_t)L2PF * n1 * n2;
+    const void* src = lane == 4 ? (const void*)(op.w + ja * g.RS)
+                    : lane == 5 ? (const void*)(op.off + ja * g.RS) : (const void*)(op.cnt + ja * 4);
+    const int bytes = rows * (lane == 4 ? g.RS * 16 : lane == 5 ? g.RS * 4 : 16);
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+  }
+  for (int chunk = cfirst; chunk < clast; ++chunk) {
+    const int m = chunk * FK_CW + lane;
+    const bool active = m >= n && m <= N;
+    const double* __restrict__ u = Pold + (size_t)chunk * chunk_elems + lane;
+    const double* __restrict__ d0 = dP + (size_t)chunk * chunk_elems + lane;
+    const double* __restrict__ d1 = d0 + field;
+    const double* __restrict__ d2 = d1 + field;
+    double* __restrict__ out = Pnew + (size_t)chunk * chunk_elems + (size_t)jb * FK_CW + lane;
+    if (!ok) {
+      // ---- row-at-a-time path
 #pragma unroll
-  for (int r = 0; r < RB; ++r)
-    if (r < rows && active) out[r * FK_CW] = acc[r];
+      for (int r = 0; r < RB; ++r) {
+        if (r < rows) {
+          const size_t j = (size_t)(jb + r);
+          const double acc = fkd::contract_row<3>(g, op.w + j * g.RS, op.off + j * g.RS, cnt[r],
+                                                  op.c[j], u, d0, d1, d2);
+          if (active) out[r * FK_CW] = acc;
+        }
+      }
+      continue;
+    }
+    // ---- blocked path
+    double acc[RB];
+    const double* __restrict__ ub = u + base2;
+    const double* __restrict__ d0b = d0 + base2;
+    const double* __restrict__ d1b = d1 + base2;
+    const double* __restrict__ d2b = d2 + base2;
+    if ((tmask & ~0x04u) == 0) contract_group<2, 2>(st, cref, ub, d0b, d1b, d2b, acc);
+    else if ((tmask & ~0x06u) == 0) contract_group<1, 2>(st, cref, ub, d0b, d1b, d2b, acc);
+    else if ((tmask & ~0x0cu) == 0) contract_group<2, 3>(st, cref, ub, d0b, d1b, d2b, acc);
+    else if ((tmask & ~0x0eu) == 0) contract_group<1, 3>(st, cref, ub, d0b, d1b, d2b, acc);
+    else contract_group<0, 4>(st, cref, ub, d0b, d1b, d2b, acc);
+#pragma unroll
+    for (int r = 0; r < RB; ++r)
+      if (r < rows && active) out[r * FK_CW] = acc[r];
+  }
 }
 
 }  // namespace
@@ -243,7 +287,7 @@ cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* P
                                  int chunk1, int n, int N, cudaStream_t s) {
   const int G2 = (g.n[2] + RB - 1) / RB;
   const int NT1 = (g.n[1] + WARPS - 1) / WARPS;
-  dim3 block(FK_CW, WARPS), grid((unsigned)((long long)g.n[0] * NT1 * G2), (unsigned)(chunk1 - chunk0));
-  fk_rowblock3d<<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, G2, NT1);
+  dim3 block(FK_CW, WARPS), grid((unsigned)((long long)g.n[0] * NT1 * G2), (unsigned)((chunk1 - chunk0 + CPB - 1) / CPB));
+  fk_rowblock3d<<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, chunk1, n, N, G2, NT1);
   return cudaGetLastError();
 }
