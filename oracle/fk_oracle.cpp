@@ -17,6 +17,8 @@
 //   ofk_apply           PAPER.md:224-229   Scheme 1 steps 1-3 = Eq. 21, 20, 22 for one field
 //   ofk_column          PAPER.md:271-273   Eq. 29: p^m = A_0 (A_1 ... (A_{m-1} chi))
 //   ofk_algorithm1      PAPER.md:277-291   Algorithm 1 (all columns, one pass)
+//   ofk_reduce          PAPER.md:62-66, 453  sum_j w_j P(t_m, x_j): the quadrature of
+//                                          int P(t,x) P_init(x) dx and of the moment of Eq. 42
 // Readings of silent / garbled points (R1..R20) are listed in DESIGN.md; the ones used here:
 //   R1 weights normalised to sum 1; R2 sigma*sqrt(2 dt)*a_q; R4 values + nodal gradient, no
 //   mixed derivatives; R5 unweighted harmonic mean; R6 end nodes use the first/last two
@@ -24,7 +26,12 @@
 //   R8 a point strictly outside an ABSORB face takes that face's value g; R9 CLAMP faces
 //   project the point onto the box first, then the lowest ABSORB dimension left outside
 //   decides g; R10 column 0 is chi; R11 coefficients at the left end t_nu; R15 Dirichlet
-//   nodes (on an ABSORB face) keep their value; R19 cell = the one with x[c] <= z < x[c+1].
+//   nodes (on an ABSORB face) keep their value; R19 cell = the one with x[c] <= z < x[c+1];
+//   R21 PERIODIC dimension ("periodic in x1"): the last node is the image of the
+//   first, a point is wrapped into [alpha, beta) before it is located, slopes use the cell across
+//   the seam; R22 slope_rule = 1: Fritsch-Carlson weighted harmonic mean (ref [17], PAPER.md:134,
+//   152-160) -- interior nodes w1 = 2 h_j + h_{j-1}, w2 = h_j + 2 h_{j-1}; the end nodes apply the
+//   same weights to their first / last two cells.
 //
 // Pins (tests/test_oracle_*.py, none of them re-types these formulas): closed-form GH rules
 // and moments; the hand-derived 5-node micro-example in tests/golden/; affine exactness;
@@ -46,7 +53,7 @@
 
 extern "C" {
 
-enum { OFK_ABSORB = 0, OFK_CLAMP = 1 };
+enum { OFK_ABSORB = 0, OFK_CLAMP = 1, OFK_PERIODIC = 2 };
 
 typedef struct {
   int d;                    // 1..3
@@ -56,6 +63,7 @@ typedef struct {
   int Q[3];                 // Gauss-Hermite points per dimension
   int face_kind[3][2];      // [dim][lo/hi]
   double face_value[3][2];  // g for ABSORB faces
+  int slope_rule;           // 0: Eq. 15 as printed (unweighted harmonic mean); 1: weighted (R22)
 } ofk_problem;
 
 // ---------------------------------------------------------------------------------------
@@ -164,15 +172,44 @@ static double harmonic(double da, double db) {
   return 2.0 / (1.0 / da + 1.0 / db);
 }
 
-int ofk_pchip_slopes(int n, const double* x, const double* u, long stride, double* du) {
+// R22: weighted harmonic mean of the divided differences da (cell of width ha) and db (cell of
+// width hb) that meet at a node: (w1 + w2) / (w1 / da + w2 / db), w1 = 2 hb + ha, w2 = hb + 2 ha.
+static double harmonic_weighted(double da, double db, double ha, double hb) {
+  bool same = (da > 0.0 && db > 0.0) || (da < 0.0 && db < 0.0);
+  if (!same) return 0.0;
+  double w1 = 2.0 * hb + ha, w2 = hb + 2.0 * ha;
+  return (w1 + w2) / (w1 / da + w2 / db);
+}
+
+static double node_slope(double da, double db, double ha, double hb, int weighted) {
+  return weighted ? harmonic_weighted(da, db, ha, hb) : harmonic(da, db);
+}
+
+// periodic != 0 (R21): node n-1 is the image of node 0, so both take the slope of the two cells
+// that meet there, the last cell (n-2) and the first (0).
+int ofk_pchip_slopes_ex(int n, const double* x, const double* u, long stride, double* du,
+                        int periodic, int weighted) {
   if (n < 3) return 1;
-  std::vector<double> delta(n - 1);
-  for (int j = 0; j < n - 1; ++j)
-    delta[j] = (u[(long)(j + 1) * stride] - u[(long)j * stride]) / (x[j + 1] - x[j]);
-  du[0] = harmonic(delta[0], delta[1]);
-  for (int j = 1; j < n - 1; ++j) du[(long)j * stride] = harmonic(delta[j - 1], delta[j]);
-  du[(long)(n - 1) * stride] = harmonic(delta[n - 2], delta[n - 3]);
+  std::vector<double> delta(n - 1), h(n - 1);
+  for (int j = 0; j < n - 1; ++j) {
+    h[j] = x[j + 1] - x[j];
+    delta[j] = (u[(long)(j + 1) * stride] - u[(long)j * stride]) / h[j];
+  }
+  for (int j = 1; j < n - 1; ++j)
+    du[(long)j * stride] = node_slope(delta[j - 1], delta[j], h[j - 1], h[j], weighted);
+  if (periodic) {
+    double s = node_slope(delta[n - 2], delta[0], h[n - 2], h[0], weighted);
+    du[0] = s;
+    du[(long)(n - 1) * stride] = s;
+  } else {
+    du[0] = node_slope(delta[0], delta[1], h[0], h[1], weighted);
+    du[(long)(n - 1) * stride] = node_slope(delta[n - 2], delta[n - 3], h[n - 2], h[n - 3], weighted);
+  }
   return 0;
+}
+
+int ofk_pchip_slopes(int n, const double* x, const double* u, long stride, double* du) {
+  return ofk_pchip_slopes_ex(n, x, u, stride, du, 0, 0);
 }
 
 // All d partial-derivative fields of u: du[k][j], slopes along the grid lines of axis k.
@@ -187,7 +224,8 @@ static void gradient_fields(const ofk_problem* p, const double* u, double* du /*
       int idx[3];
       unravel(p, j, idx);
       if (idx[k] != 0) continue;                     // j is the first node of a line along k
-      ofk_pchip_slopes(p->n[k], p->x[k], u + j, st[k], dk + j);
+      ofk_pchip_slopes_ex(p->n[k], p->x[k], u + j, st[k], dk + j,
+                          p->face_kind[k][0] == OFK_PERIODIC, p->slope_rule);
     }
   }
 }
@@ -298,6 +336,15 @@ static void apply_with_rule(const ofk_problem* p, const double* b, const double*
       }
       for (int k = 0; k < d; ++k) {                                 // R9: CLAMP faces first
         double lo = p->x[k][0], hi = p->x[k][p->n[k] - 1];
+        if (p->face_kind[k][0] == OFK_PERIODIC) {                   // R21: wrap into [lo, hi)
+          if (z[k] < lo || z[k] >= hi) {
+            double L = hi - lo;
+            double r = std::fmod(z[k] - lo, L);
+            if (r < 0.0) r += L;
+            z[k] = lo + r;
+          }
+          continue;
+        }
         if (z[k] < lo && p->face_kind[k][0] == OFK_CLAMP) z[k] = lo;
         if (z[k] > hi && p->face_kind[k][1] == OFK_CLAMP) z[k] = hi;
       }
@@ -375,6 +422,19 @@ int ofk_algorithm1(const ofk_problem* p, const double* b_tab, const double* s_ta
       apply_with_rule(p, b_tab + off, s_tab + off, rule.ap, rule.wp, col, v.data(), du.data());
       std::memcpy(col, v.data(), sizeof(double) * J);
     }
+  }
+  return 0;
+}
+
+// sum_j w_j P(t_m, x_j) for M columns stored as P[M][J] (the exit probability
+// for initial conditions distributed as P_init is int P(t,x) P_init(x) dx -- w_j = quadrature
+// weight times P_init(x_j); Eq. 42: the same with w_j = 2 pi n_0 f_M(p_j) times the
+// (xi, p) quadrature weights on the slice r = r_0).  Plain definition, long-double sum.
+int ofk_reduce(long J, int M, const double* P, const double* w, double* out) {
+  for (int m = 0; m < M; ++m) {
+    long double s = 0.0L;
+    for (long j = 0; j < J; ++j) s += (long double)w[j] * (long double)P[(long)m * J + j];
+    out[m] = (double)s;
   }
   return 0;
 }

@@ -29,7 +29,7 @@ def build(force: bool = False) -> str:
 class _Problem(C.Structure):
     _fields_ = [("d", C.c_int), ("n", C.c_int * 3), ("x", C.POINTER(C.c_double) * 3),
                 ("dt", C.c_double), ("Q", C.c_int * 3), ("face_kind", (C.c_int * 2) * 3),
-                ("face_value", (C.c_double * 2) * 3)]
+                ("face_value", (C.c_double * 2) * 3), ("slope_rule", C.c_int)]
 
 
 _lib = None
@@ -44,6 +44,8 @@ def lib():
         _lib.ofk_gauss_hermite.argtypes = [C.c_int, dp, dp]
         _lib.ofk_chi.argtypes = [pp, dp]
         _lib.ofk_pchip_slopes.argtypes = [C.c_int, dp, dp, C.c_long, dp]
+        _lib.ofk_pchip_slopes_ex.argtypes = [C.c_int, dp, dp, C.c_long, dp, C.c_int, C.c_int]
+        _lib.ofk_reduce.argtypes = [C.c_long, C.c_int, dp, dp, dp]
         _lib.ofk_interp.argtypes = [pp, dp, C.c_long, dp, dp]
         _lib.ofk_apply.argtypes = [pp, dp, dp, dp, dp]
         _lib.ofk_column.argtypes = [pp, dp, dp, C.c_int, C.c_int, dp]
@@ -81,6 +83,7 @@ class Oracle:
                 p.face_kind[k][s] = int(wl.face_kind[k][s])
                 p.face_value[k][s] = float(wl.face_value[k][s])
         p.dt = float(wl.dt)
+        p.slope_rule = int(getattr(wl, "slope_rule", 0))
         self.p = p
         self.J = wl.J
 
@@ -149,10 +152,19 @@ def gauss_hermite(Q):
     return a, w
 
 
-def pchip_slopes(x, u):
+def reduce(P, w):
+    """sum_j w_j P[m][j] for every row m of P."""
+    P, w = _f64(P), _f64(w)
+    P = P.reshape(-1, w.size)
+    out = np.empty(P.shape[0])
+    lib().ofk_reduce(w.size, P.shape[0], _ptr(P), _ptr(w), _ptr(out))
+    return out
+
+
+def pchip_slopes(x, u, periodic=False, weighted=False):
     x, u = _f64(x), _f64(u)
     du = np.empty_like(u)
-    rc = lib().ofk_pchip_slopes(len(x), _ptr(x), _ptr(u), 1, _ptr(du))
+    rc = lib().ofk_pchip_slopes_ex(len(x), _ptr(x), _ptr(u), 1, _ptr(du), int(periodic), int(weighted))
     if rc:
         raise ValueError("need at least 3 nodes")
     return du

@@ -23,6 +23,9 @@ import numpy as np
 
 FACE_ABSORB = 0
 FACE_CLAMP = 1
+FACE_PERIODIC = 2
+SLOPE_EQ15 = 0        # Eq. 15 as printed: unweighted harmonic mean
+SLOPE_WEIGHTED = 1    # Fritsch-Carlson weighted harmonic mean (ref [17]) for non-uniform grids
 
 
 @dataclass
@@ -32,7 +35,8 @@ class Workload:
     x[k]        node coordinates along dimension k (strictly increasing, ends = box faces)
     dt, N       uniform time partition, T_max = N*dt (Eq. 10)
     Q[k]        Gauss-Hermite points along dimension k
-    face_kind   [d][2] FACE_ABSORB / FACE_CLAMP for the (lo, hi) face of each dimension
+    face_kind   [d][2] FACE_ABSORB / FACE_CLAMP / FACE_PERIODIC (both faces of a dimension)
+    slope_rule  SLOPE_EQ15 or SLOPE_WEIGHTED
     face_value  [d][2] value g taken by a point leaving through an ABSORB face (1 = "exit")
     coeffs(n)   -> (b, sigma), float64 arrays [d][J], sampled at t_n = n*dt
     autonomous  True when coeffs(n) does not depend on n
@@ -49,6 +53,7 @@ class Workload:
     autonomous: bool = False
     note: str = ""
     extra: dict = field(default_factory=dict)
+    slope_rule: int = SLOPE_EQ15
 
     @property
     def d(self) -> int:
@@ -227,14 +232,24 @@ def runaway_2d(n=(401, 201), N: int = 5000, T_max: float = 120.0, Q=(8, 8),
                     note="p in [0,50] exit at p_max (g=1), p=0 g=0, xi faces clamp; E ramp")
 
 
+def radial_grid(coarse: int = 7, fine: int = 120, r_D: float = 0.7) -> np.ndarray:
+    """The paper's non-uniform radial grid (Fig. 8): spacing r_D / coarse (0.1) on
+    [0, r_D] and (1 - r_D) / fine (0.0025) on [r_D, 1]: coarse + fine + 1 nodes."""
+    return np.concatenate([np.linspace(0.0, r_D, coarse + 1)[:-1], np.linspace(r_D, 1.0, fine + 1)])
+
+
 def runaway_3d(n=(161, 81, 65), N: int = 2000, T_max: float = 120.0, Q=(6, 6, 6),
                p_max: float = 50.0, seed: int = 20210414, dt: Optional[float] = None,
                r_D: float = 0.7, W: float = 1e-2, dp: float = 20.0, V0: float = 0.003,
-               D0: float = 1e-4) -> Workload:
-    """(p, xi, r) of Eq. 37-38 with E(t, r) = E_amp(t) (1 - r^2/2), seeded random-amplitude ramp."""
+               D0: float = 1e-4, xr: Optional[np.ndarray] = None,
+               slope_rule: int = SLOPE_EQ15) -> Workload:
+    """(p, xi, r) of Eq. 37-38 with E(t, r) = E_amp(t) (1 - r^2/2), seeded random-amplitude ramp.
+    xr: radial nodes (default uniform, n[2] of them); radial_grid() gives the paper's
+    piecewise-uniform grid."""
     xp = np.linspace(0.0, p_max, n[0])
     xx = np.linspace(-1.0, 1.0, n[1])
-    xr = np.linspace(0.0, 1.0, n[2])
+    xr = np.linspace(0.0, 1.0, n[2]) if xr is None else np.asarray(xr, dtype=np.float64)
+    n = (n[0], n[1], len(xr))
     dt = T_max / N if dt is None else dt
     P, XI, R = np.meshgrid(xp, xx, xr, indexing="ij")
     P = P.reshape(-1)
@@ -272,15 +287,67 @@ def runaway_3d(n=(161, 81, 65), N: int = 2000, T_max: float = 120.0, Q=(6, 6, 6)
                          [[0.0, 1.0], [0.0, 0.0], [0.0, 0.0]])
     return Workload("cfg5_runaway_3d", (xp, xx, xr), dt, N, tuple(Q), kinds, vals, coeffs,
                     note="as cfg4 + radial row; r=0 clamp, r=1 absorb g=0; seeded E knots",
-                    extra={"E_amp": E_amp, "parts": (bp0, bpE, bx0, bxE, br)})
+                    extra={"E_amp": E_amp, "parts": (bp0, bpE, bx0, bxE, br)},
+                    slope_rule=slope_rule)
+
+
+# --------------------------------------------------------------------------------------
+# the paper's own 2-D example: cellular flow, periodic in x1 (Eq. 32-36)
+# --------------------------------------------------------------------------------------
+def cellular_periodic_2d(n=(129, 65), N: int = 100, T_max: float = 0.05, Q=(4, 4),
+                         Pe: float = 10.0, eps: float = 0.15, omega: float = 2.0 * math.pi / 10.0,
+                         cells: int = 2, dt: Optional[float] = None) -> Workload:
+    """dx = Pe v(x, t) dt + dW on [-pi, pi] x [0, 1] with v of Eq. 33-35 (f = cos(omega t)),
+    periodic in x1, P = 1 on x2 = 0 and x2 = 1 (Pe = 10, eps = 0.15,
+    omega = 2 pi / 10, n = 2, T_max = 0.05).  The paper gives no grid or step count for this
+    example in its text: 129 x 65 nodes and N = 100 are this repo's choice."""
+    x0 = np.linspace(-math.pi, math.pi, n[0])
+    x1 = np.linspace(0.0, 1.0, n[1])
+    dt = T_max / N if dt is None else dt
+    X, Y = np.meshgrid(x0, x1, indexing="ij")
+    X = X.reshape(-1)
+    Y = Y.reshape(-1)
+    J = X.size
+    snx, cnx = np.sin(cells * X), np.cos(cells * X)
+    cpy, spy = np.cos(math.pi * Y), np.sin(math.pi * Y)
+    # the last x1 node is the image of the first: give both exactly the same coefficients
+    first = np.arange(J).reshape(n)[0]
+    last = np.arange(J).reshape(n)[-1]
+    sig = np.ones((2, J))
+
+    def coeffs(nstep):
+        f = math.cos(omega * nstep * dt)
+        b = np.empty((2, J))
+        b[0] = Pe * (-math.pi * cpy * (snx + eps * f * cnx))
+        b[1] = Pe * (cells * spy * (cnx - eps * f * snx))
+        b[:, last] = b[:, first]
+        return b, sig
+
+    kinds, vals = _faces([[FACE_PERIODIC, FACE_PERIODIC], [FACE_ABSORB, FACE_ABSORB]],
+                         [[0.0, 0.0], [1.0, 1.0]])
+    return Workload("cfg6_cellular_periodic_2d", (x0, x1), dt, N, tuple(Q), kinds, vals, coeffs,
+                    note="paper's Eq. 33-36: Pe=10, eps=0.15, omega=2pi/10, n=2; periodic x1")
 
 
 # --------------------------------------------------------------------------------------
 # registry: full-size configs (BASELINE.json order) and reduced shapes for parity tests
 # --------------------------------------------------------------------------------------
+def runaway_3d_radial(**kw) -> Workload:
+    """Config 5 on the paper's non-uniform radial grid (0.1 / 0.0025 spacing) with
+    the weighted harmonic mean of ref [17]."""
+    kw.setdefault("xr", radial_grid())
+    kw.setdefault("slope_rule", SLOPE_WEIGHTED)
+    wl = runaway_3d(**kw)
+    wl.name = "cfg7_runaway_3d_radial"
+    return wl
+
+
 def config(idx: int, **kw) -> Workload:
-    """BASELINE.json config `idx` in 1..5 at full size; keyword overrides shrink it."""
-    return {1: brownian_1d, 2: ou_1d, 3: cellular_2d, 4: runaway_2d, 5: runaway_3d}[idx](**kw)
+    """BASELINE.json config `idx` in 1..5 at full size; keyword overrides shrink it.  6 and 7 are
+    the SURVEY.md section 8(f) workloads: the paper's periodic cellular flow and the runaway
+    problem on the paper's non-uniform radial grid."""
+    return {1: brownian_1d, 2: ou_1d, 3: cellular_2d, 4: runaway_2d, 5: runaway_3d,
+            6: cellular_periodic_2d, 7: runaway_3d_radial}[idx](**kw)
 
 
 def small(idx: int) -> Workload:
@@ -295,6 +362,10 @@ def small(idx: int) -> Workload:
         return runaway_2d(n=(83, 47), N=33, dt=120.0 / 5000)
     if idx == 5:
         return runaway_3d(n=(37, 23, 19), N=19, dt=120.0 / 2000)
+    if idx == 6:
+        return cellular_periodic_2d(n=(41, 27), N=35, dt=0.05 / 100)
+    if idx == 7:
+        return runaway_3d_radial(n=(29, 19, 0), N=13, dt=120.0 / 2000, xr=radial_grid(3, 20))
     raise KeyError(idx)
 
 
