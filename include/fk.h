@@ -43,15 +43,24 @@ enum { FK_OK = 0, FK_EINVAL = 1, FK_ENOMEM = 2, FK_ECUDA = 3, FK_ESTATE = 4 };
  *         face are updated like interior nodes.
  * CLAMP dimensions are projected first; among the remaining dimensions that are outside, the
  * lowest dimension index decides the value. */
-enum { FK_FACE_ABSORB = 0, FK_FACE_CLAMP = 1 };
+/* PERIODIC (both faces of a dimension or neither; R21; "periodic in x1"):
+ *         x[k][n-1] is the image of x[k][0] one period L = beta - alpha later; a point is
+ *         wrapped into [alpha, beta) before it is located; Eq. 15 uses the cell across the seam
+ *         at the first / last node; both end nodes are updated like interior nodes (give them the
+ *         same coefficients).  Problems with a periodic dimension run on the generic kernels. */
+enum { FK_FACE_ABSORB = 0, FK_FACE_CLAMP = 1, FK_FACE_PERIODIC = 2 };
 
 enum { FK_MEM_HOST = 0, FK_MEM_DEVICE = 1 };
 
 /* fk_params.flags */
 enum {
-  FK_FLAG_VALIDATE = 1   /* check every coefficient read by an updated node for NaN / Inf on the
+  FK_FLAG_VALIDATE = 1,  /* check every coefficient read by an updated node for NaN / Inf on the
                             device while the operator is assembled (costs two compares per
                             value); a hit is reported like a negative sigma, see fk_check */
+  FK_FLAG_WEIGHTED_SLOPES = 2  /* nodal slopes by the Fritsch-Carlson weighted harmonic mean
+                            (ref [17]; R22) instead of Eq. 15 as printed:
+                            (w1+w2)/(w1/d_{j-1} + w2/d_j), w1 = 2h_j + h_{j-1}, w2 = h_j + 2h_{j-1};
+                            equal to Eq. 15 on uniform grids, meant for non-uniform ones */
 };
 
 #define FK_ALL_STEPS (-1)
@@ -77,6 +86,11 @@ typedef struct {
   int device;              /* CUDA device ordinal (compute capability 10.x) */
   void* stream;            /* cudaStream_t (e.g. from torch); NULL = the legacy default stream */
   unsigned flags;          /* FK_FLAG_* or 0 */
+  int shard_index;         /* column sharding (the columns are independent): this */
+  int shard_count;         /* context keeps and updates only the 32-column chunks c with
+                              c % shard_count == shard_index; 0 or 1 = all columns.  Shards never
+                              exchange data; fk_read / fk_reduce of a shard write only the columns
+                              it owns and leave the other entries of `out` untouched */
 } fk_params;
 
 /* Validate, build the Gauss-Hermite tables, allocate device state and fill both P buffers
@@ -122,6 +136,16 @@ int fk_reset(fk_ctx* c);
  * that only column 0 and, after reaching n, nothing else is final (FK_ESTATE).  The call
  * synchronises the stream when `mem` is FK_MEM_HOST. */
 int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem);
+
+/* Weighted reduction over the nodes of every requested column, straight from the device layout:
+ * out[m - m0] = sum_j weights[j] * P(t_m, x_j) for m0 <= m < m1 (weights[J] and out[m1-m0] in
+ * host or device memory, same kind `mem` for both).  With w_j = (quadrature weight of node j) *
+ * P_init(x_j) this is the exit probability for initial conditions distributed as P_init,
+ * int P(t,x) P_init(x) dx; with w_j = 2 pi n_0 f_M(p_j) * (quadrature weight)
+ * on the nodes of the slice r = r_0 and 0 elsewhere it is the moment n_RE(r_0, t) of Eq. 42
+ * (PAPER.md:453).  The sum over nodes runs in a fixed order (reproducible).  State rules as
+ * fk_read; synchronises the stream when `mem` is FK_MEM_HOST. */
+int fk_reduce(fk_ctx* c, const double* weights, int m0, int m1, double* out, int mem);
 
 /* Synchronise the context's stream and report what the device found since the last fk_reset:
  * FK_OK, or FK_EINVAL with fk_last_error naming the first kind of bad coefficient (negative

@@ -1,7 +1,7 @@
 """ctypes binding of the C ABI in include/fk.h (libfk_b200.so): argument marshalling only.
 
 Same names as the C entry points (`fk_create`, `fk_set_coeffs`, `fk_set_coeffs_range`,
-`fk_evolve`, `fk_reset`, `fk_read`, `fk_check`, `fk_profile`, `fk_profile_read`,
+`fk_evolve`, `fk_reset`, `fk_read`, `fk_reduce`, `fk_check`, `fk_profile`, `fk_profile_read`,
 `fk_launch_count`, `fk_destroy`, `fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
 pointers) or torch CUDA tensors (device pointers); every step of the path runs in the CUDA
 kernels behind the ABI.  There is no CPU fallback: a missing library raises.
@@ -14,18 +14,19 @@ import os
 import numpy as np
 
 FK_OK, FK_EINVAL, FK_ENOMEM, FK_ECUDA, FK_ESTATE = 0, 1, 2, 3, 4
-FK_FACE_ABSORB, FK_FACE_CLAMP = 0, 1
+FK_FACE_ABSORB, FK_FACE_CLAMP, FK_FACE_PERIODIC = 0, 1, 2
 FK_MEM_HOST, FK_MEM_DEVICE = 0, 1
 FK_ALL_STEPS = -1
 FK_MAX_Q = 32
 FK_FLAG_VALIDATE = 1
+FK_FLAG_WEIGHTED_SLOPES = 2
 FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_ROWBLOCK, FK_K_COUNT = 0, 1, 2, 3, 4, 5
 KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock")
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 
 EXPORTS = ("fk_create", "fk_set_coeffs", "fk_set_coeffs_range", "fk_evolve", "fk_reset",
-           "fk_read", "fk_check", "fk_profile", "fk_profile_read", "fk_launch_count", "fk_destroy",
+           "fk_read", "fk_reduce", "fk_check", "fk_profile", "fk_profile_read", "fk_launch_count", "fk_destroy",
            "fk_last_error", "fk_gauss_hermite")
 
 
@@ -40,7 +41,7 @@ class fk_params(C.Structure):
                 ("dt", C.c_double), ("N", C.c_int), ("Q", C.c_int * 3),
                 ("face_kind", (C.c_int * 2) * 3), ("face_value", (C.c_double * 2) * 3),
                 ("coeff_slots", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
-                ("flags", C.c_uint)]
+                ("flags", C.c_uint), ("shard_index", C.c_int), ("shard_count", C.c_int)]
 
 
 _lib = None
@@ -62,6 +63,7 @@ def lib():
         L.fk_evolve.argtypes = [vp, C.c_int, C.c_int]
         L.fk_reset.argtypes = [vp]
         L.fk_read.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
+        L.fk_reduce.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int]
         L.fk_check.argtypes = [vp]
         L.fk_profile.argtypes = [vp, C.c_int]
         L.fk_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
@@ -106,7 +108,8 @@ def fk_gauss_hermite(Q):
     return a, w
 
 
-def fk_create(x, dt, N, Q, face_kind, face_value, coeff_slots=0, device=0, stream=0, flags=0):
+def fk_create(x, dt, N, Q, face_kind, face_value, coeff_slots=0, device=0, stream=0, flags=0,
+              shard_index=0, shard_count=1):
     """-> opaque context handle.  x: list of d node arrays; Q, face_kind[d][2], face_value[d][2]."""
     p = fk_params()
     d = len(x)
@@ -127,6 +130,8 @@ def fk_create(x, dt, N, Q, face_kind, face_value, coeff_slots=0, device=0, strea
     p.device = int(device)
     p.stream = C.c_void_p(int(stream) or None)
     p.flags = int(flags)
+    p.shard_index = int(shard_index)
+    p.shard_count = int(shard_count)
     ctx = C.c_void_p()
     rc = lib().fk_create(C.byref(p), C.byref(ctx))
     if rc != FK_OK:
@@ -164,6 +169,19 @@ def fk_read(ctx, m0, m1, out):
     if ko is not out:
         raise TypeError("out must be a C-contiguous float64 numpy array or torch tensor")
     _check(ctx, lib().fk_read(ctx, int(m0), int(m1), po, mo))
+    return out
+
+
+def fk_reduce(ctx, weights, m0, m1, out):
+    """out[m - m0] = sum_j weights[j] P(t_m, x_j); weights [J] and out [m1-m0] both numpy arrays or
+    both CUDA tensors."""
+    pw, mw, kw = _buffer(weights)
+    po, mo, ko = _buffer(out, m1 - m0)
+    if ko is not out:
+        raise TypeError("out must be a C-contiguous float64 numpy array or torch tensor")
+    if mw != mo:
+        raise ValueError("weights and out must both be host or both be device arrays")
+    _check(ctx, lib().fk_reduce(ctx, pw, int(m0), int(m1), po, mo))
     return out
 
 

@@ -22,7 +22,12 @@ struct EventPair { cudaEvent_t a, b; int cls; };
 
 struct fk_ctx {
   FkGrid g;
-  int N = 0, slots = 0, device = 0, n_chunks = 0;
+  int N = 0, slots = 0, device = 0;
+  int n_chunks = 0;                    // chunks this context owns (all of them unless sharded)
+  bool fused2d = false;                // 2-D: near rows go through fk_fused2d (else generic only)
+  double2* d_wgt[3] = {nullptr, nullptr, nullptr};
+  double* d_red = nullptr;             // fk_reduce: weights [J], partial sums, result
+  size_t red_bytes = 0;
   cudaStream_t stream = nullptr;
   double* d_x[3] = {nullptr, nullptr, nullptr};
   double* d_invh[3] = {nullptr, nullptr, nullptr};
@@ -142,7 +147,8 @@ void gauss_hermite(int Q, double* a, double* w) {
 void release(fk_ctx* c) {
   if (!c) return;
   DeviceGuard guard(c->device);
-  for (int k = 0; k < 3; ++k) { cudaFree(c->d_x[k]); cudaFree(c->d_invh[k]); }
+  for (int k = 0; k < 3; ++k) { cudaFree(c->d_x[k]); cudaFree(c->d_invh[k]); cudaFree(c->d_wgt[k]); }
+  cudaFree(c->d_red);
   cudaFree(c->d_coef);
   cudaFree(c->raw_P[0]);
   cudaFree(c->raw_P[1]);
@@ -201,8 +207,11 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     for (int i = 0; i < p->n[k]; ++i)
       if (!std::isfinite(p->x[k][i]) || (i > 0 && !(p->x[k][i] > p->x[k][i - 1])))
         return fail(nullptr, FK_EINVAL, "x[k] must be finite and strictly increasing");
+    if ((p->face_kind[k][0] == FK_FACE_PERIODIC) != (p->face_kind[k][1] == FK_FACE_PERIODIC))
+      return fail(nullptr, FK_EINVAL, "FK_FACE_PERIODIC must be set on both faces of a dimension");
     for (int s = 0; s < 2; ++s) {
-      if (p->face_kind[k][s] != FK_FACE_ABSORB && p->face_kind[k][s] != FK_FACE_CLAMP)
+      if (p->face_kind[k][s] != FK_FACE_ABSORB && p->face_kind[k][s] != FK_FACE_CLAMP &&
+          p->face_kind[k][s] != FK_FACE_PERIODIC)
         return fail(nullptr, FK_EINVAL, "unknown face_kind");
       if (p->face_kind[k][s] == FK_FACE_ABSORB && !std::isfinite(p->face_value[k][s]))
         return fail(nullptr, FK_EINVAL, "face_value of an ABSORB face must be finite");
@@ -222,7 +231,11 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   if (cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, p->device) != cudaSuccess ||
       cc_major != 10)
     return fail(nullptr, FK_ECUDA, "device is not compute capability 10.x: the kernels are built for sm_100a only");
-  if (p->flags & ~(unsigned)FK_FLAG_VALIDATE) return fail(nullptr, FK_EINVAL, "unknown bits in flags");
+  if (p->flags & ~(unsigned)(FK_FLAG_VALIDATE | FK_FLAG_WEIGHTED_SLOPES))
+    return fail(nullptr, FK_EINVAL, "unknown bits in flags");
+  const int shard_count = p->shard_count <= 0 ? 1 : p->shard_count;
+  if (p->shard_index < 0 || p->shard_index >= shard_count)
+    return fail(nullptr, FK_EINVAL, "need 0 <= shard_index < shard_count");
   DeviceGuard guard(p->device);
 
   fk_ctx* c = new (std::nothrow) fk_ctx();
@@ -231,7 +244,11 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   c->stream = (cudaStream_t)p->stream;
   c->N = p->N;
   c->slots = slots;
-  c->n_chunks = p->N / FK_CW + 1;          // columns 0..N
+  {
+    const int all = p->N / FK_CW + 1;       // columns 0..N; this shard owns c = index, index+count, ...
+    c->n_chunks = all > p->shard_index ? (all - p->shard_index + shard_count - 1) / shard_count : 0;
+    if (c->n_chunks == 0) { delete c; return fail(nullptr, FK_EINVAL, "this shard owns no column: shard_count exceeds the number of 32-column chunks"); }
+  }
   c->n_next = p->N;
   c->slot_step.assign(slots, -2);
 
@@ -242,6 +259,9 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   g.dt = p->dt;
   g.sq = std::sqrt(2.0 * p->dt);
   g.validate = (p->flags & FK_FLAG_VALIDATE) ? 1 : 0;
+  g.weighted = (p->flags & FK_FLAG_WEIGHTED_SLOPES) ? 1 : 0;
+  g.shard_index = p->shard_index;
+  g.shard_count = shard_count;
   int qoff = 0;
   for (int k = 0; k < 3; ++k) { g.n[k] = 1; g.Q[k] = 0; g.stride[k] = 0; }
   long long st = 1;
@@ -259,6 +279,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     for (int i = 0; i < p->n[k]; ++i)
       if (std::fabs(p->x[k][i] - (g.lo[k] + i * h0)) > 1e-9 * h0) uniform = 0;
     g.uniform[k] = uniform;
+    g.periodic[k] = p->face_kind[k][0] == FK_FACE_PERIODIC;
     for (int s = 0; s < 2; ++s) {
       g.face_kind[k][s] = p->face_kind[k][s];
       g.face_value[k][s] = p->face_value[k][s];
@@ -288,6 +309,34 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     FK_CREATE_CUDA(cudaStreamSynchronize(c->stream));   // ih is a local
     g.x[k] = c->d_x[k];
     g.inv_h[k] = c->d_invh[k];
+    if (g.weighted) {
+      // R22: per node the weights attached to the two divided differences of its slope window
+      // (fk_kernels.cu slope_window): cells (ca, cb) of widths (ha, hb); the difference of ca
+      // carries w = 2 hb + ha, that of cb carries hb + 2 ha -- except at the last node of a
+      // non-periodic line, where the window is read in the opposite order (delta_{n-2} first)
+      std::vector<double2> wg(n);
+      for (int i = 0; i < n; ++i) {
+        int ca, cb;
+        if (g.periodic[k]) { ca = i == 0 ? n - 2 : i - 1; cb = i == n - 1 ? 0 : i; }
+        else { const int la = i - 1 < 0 ? 0 : (i - 1 > n - 3 ? n - 3 : i - 1); ca = la; cb = la + 1; }
+        const double ha = p->x[k][ca + 1] - p->x[k][ca], hb = p->x[k][cb + 1] - p->x[k][cb];
+        double wa = 2.0 * hb + ha, wb = hb + 2.0 * ha;
+        if (!g.periodic[k] && i == n - 1) { wa = ha + 2.0 * hb; wb = 2.0 * ha + hb; }
+        wg[i] = make_double2(wa / (wa + wb), wb / (wa + wb));
+      }
+      FK_CREATE_CUDA(cudaMalloc(&c->d_wgt[k], sizeof(double2) * n));
+      FK_CREATE_CUDA(cudaMemcpyAsync(c->d_wgt[k], wg.data(), sizeof(double2) * n, cudaMemcpyHostToDevice, c->stream));
+      FK_CREATE_CUDA(cudaStreamSynchronize(c->stream));   // wg is a local
+      g.wgt[k] = c->d_wgt[k];
+    }
+  }
+  {
+    bool any_periodic = false, all_uniform = true;
+    for (int k = 0; k < p->d; ++k) { any_periodic = any_periodic || g.periodic[k]; all_uniform = all_uniform && g.uniform[k]; }
+    g.general_slopes = (any_periodic || g.weighted) ? 1 : 0;
+    // the fused 2-D kernel computes Eq. 15 itself, for box problems: periodic dimensions and the
+    // weighted mean on a non-uniform grid go through the generic slopes / apply kernels
+    c->fused2d = p->d == 2 && !any_periodic && !(g.weighted && !all_uniform);
   }
   const size_t buf = sizeof(double) * (size_t)c->n_chunks * J * FK_CW;
   // P and dP carry FK_GUARD_ROWS zeroed 256-byte rows at both ends, and dP is cleared once: the
@@ -318,7 +367,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   FK_CREATE_CUDA(cudaHostAlloc(&c->h_status, sizeof(int), cudaHostAllocDefault));
   *c->h_status = 0;
   FK_CREATE_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
-  if (p->d == 2) {                       // the fused 2-D kernel's records and step classification
+  if (c->fused2d) {                      // the fused 2-D kernel's records and step classification
     for (int i = 0; i < 2; ++i) {
       FK_CREATE_CUDA(cudaMalloc(&c->op[i].rec, sizeof(FkRec2) * (size_t)J));
       FK_CREATE_CUDA(cudaMemsetAsync(c->op[i].rec, 0, sizeof(FkRec2) * (size_t)J, c->stream));
@@ -369,7 +418,7 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
     c->slot_step[slot] = step;
   }
   c->autonomous = false;
-  if (c->g.d == 2) {                     // which of these steps have rows outside the fused halo
+  if (c->fused2d) {                      // which of these steps have rows outside the fused halo
     const int s0 = step0 % c->slots;
     const int first = count < c->slots - s0 ? count : c->slots - s0;
     FK_CUDA(c, cudaMemsetAsync(c->d_far + (size_t)s0 * FK_FAR_STRIDE, 0, sizeof(int) * (size_t)first * FK_FAR_STRIDE, c->stream));
@@ -395,7 +444,7 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   FK_CUDA(c, cudaMemcpyAsync(c->d_coef + slice, sigma, sizeof(double) * slice, kind, c->stream));
   std::fill(c->slot_step.begin(), c->slot_step.end(), -2);
   c->autonomous = true;
-  if (c->g.d == 2) {
+  if (c->fused2d) {
     FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * FK_FAR_STRIDE, c->stream));
     FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, 0, 1, c->d_far, c->stream));
     ++c->launches;
@@ -443,7 +492,7 @@ const char* status_text(int bits) {
 // update columns n..N on the caller's stream
 int evolve_step(fk_ctx* c, int n) {
   const size_t slice = (size_t)c->g.d * c->g.J;
-  const int last_chunk = c->N / FK_CW + 1;             // one past the chunk of column N
+  const int last_chunk = c->n_chunks;                  // one past the (local) chunk of column N
   const int nu = n - 1;
   int slot = 0;
   if (!c->autonomous) {
@@ -455,9 +504,12 @@ int evolve_step(fk_ctx* c, int n) {
     }
   }
   const double* b = c->d_coef + (size_t)slot * 2 * slice;
-  const int chunk0 = n / FK_CW;                        // first chunk with an active column
+  // first local chunk with an active column: local chunk l is global chunk l * count + index
+  int chunk0 = (n / FK_CW - c->g.shard_index + c->g.shard_count - 1) / c->g.shard_count;
+  if (n / FK_CW < c->g.shard_index) chunk0 = 0;
   const double* Pold = c->d_P[c->cur];
   double* Pnew = c->d_P[c->cur ^ 1];
+  if (chunk0 >= last_chunk) return FK_OK;              // (sharded) none of this context's columns is active yet
   // assemble A_nu into buffer n & 1 on the side stream as soon as the kernels of step n + 2
   // (the buffer's previous users) are done; the kernels of this step wait for it
   const int ob = n & 1;
@@ -468,7 +520,7 @@ int evolve_step(fk_ctx* c, int n) {
     return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->side); }));
   FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
   FK_CUDA(c, cudaStreamWaitEvent(st, c->ev_ready[ob], 0));
-  const bool fused = c->g.d == 2;
+  const bool fused = c->fused2d;
   const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
   const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
   if (fused)
@@ -516,7 +568,7 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   if (n_to < 0 || n_to > n_from) return fail(c, FK_EINVAL, "need 0 <= n_to <= n_from");
   if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
   DeviceGuard guard(c->device);
-  if (c->g.d == 2 && !c->far_valid && n_from > n_to) { // one small read-back per coefficient load
+  if (c->fused2d && !c->far_valid && n_from > n_to) {  // one small read-back per coefficient load
     FK_CUDA(c, cudaMemcpyAsync(c->h_far.data(), c->d_far, sizeof(int) * (size_t)c->slots * FK_FAR_STRIDE,
                                cudaMemcpyDeviceToHost, c->stream));
     FK_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -565,11 +617,13 @@ int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem) {
     return FK_OK;
   }
   // host destination: gather into a bounded device staging buffer, copy out batch by batch
+  // (a shard copies chunk by chunk, its own chunks only: the other rows of `out` are not its)
+  const bool sharded = c->g.shard_count > 1;
   const size_t want = (size_t)256 << 20;
   int batch = (int)(want / col);
-  if (batch < FK_CW) batch = FK_CW;
+  if (batch < FK_CW || sharded) batch = FK_CW;
   batch -= batch % FK_CW;
-  if (batch > m1 - m0) batch = m1 - m0;
+  if (batch > m1 - m0 && !sharded) batch = m1 - m0;
   if (c->stage_bytes < (size_t)batch * col) {
     cudaFree(c->d_stage);
     c->d_stage = nullptr;
@@ -577,15 +631,60 @@ int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem) {
     FK_CUDA(c, cudaMalloc(&c->d_stage, (size_t)batch * col));
     c->stage_bytes = (size_t)batch * col;
   }
-  for (int a = m0; a < m1; a += batch) {
-    const int e = a + batch < m1 ? a + batch : m1;
+  for (int a = m0; a < m1;) {
+    int e = a + batch < m1 ? a + batch : m1;
+    if (sharded) {                                       // [a, e) = the part of one chunk inside [m0, m1)
+      e = (a / FK_CW + 1) * FK_CW < m1 ? (a / FK_CW + 1) * FK_CW : m1;
+      if ((a / FK_CW) % c->g.shard_count != c->g.shard_index) { a = e; continue; }
+    }
     FK_CUDA(c, fk_launch_gather_columns(c->g, P, a, e, c->d_stage, c->stream));
     ++c->launches;
     FK_CUDA(c, cudaMemcpyAsync(out + (size_t)(a - m0) * c->g.J, c->d_stage, (size_t)(e - a) * col,
                                cudaMemcpyDeviceToHost, c->stream));
     FK_CUDA(c, cudaStreamSynchronize(c->stream));
+    a = e;
   }
   if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));   // refreshed by fk_evolve
+  return FK_OK;
+}
+
+int fk_reduce(fk_ctx* c, const double* weights, int m0, int m1, double* out, int mem) {
+  if (!c) return FK_EINVAL;
+  if (!weights || !out) return fail(c, FK_EINVAL, "weights or out is NULL");
+  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
+  if (m0 < 0 || m1 > c->N + 1 || m0 >= m1) return fail(c, FK_EINVAL, "need 0 <= m0 < m1 <= N+1");
+  if (c->n_next != 0 && m1 > 1) return fail(c, FK_ESTATE, "columns other than 0 are final only after fk_evolve reached n_to = 0");
+  if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
+  DeviceGuard guard(c->device);
+  const size_t J = (size_t)c->g.J;
+  const int chunks = (m1 - 1) / FK_CW - m0 / FK_CW + 1;
+  // scratch: [J] weights (host sources), [chunks][FK_RED_BLOCKS][32] partial sums, [m1-m0] result
+  const size_t need = sizeof(double) * (J + (size_t)chunks * FK_RED_BLOCKS * FK_CW + (size_t)(m1 - m0));
+  if (c->red_bytes < need) {
+    cudaFree(c->d_red);
+    c->d_red = nullptr;
+    c->red_bytes = 0;
+    FK_CUDA(c, cudaMalloc(&c->d_red, need));
+    c->red_bytes = need;
+  }
+  double* d_w = c->d_red;
+  double* d_partial = d_w + J;
+  double* d_out = d_partial + (size_t)chunks * FK_RED_BLOCKS * FK_CW;
+  const double* w = weights;
+  if (mem == FK_MEM_HOST) {
+    FK_CUDA(c, cudaMemcpyAsync(d_w, weights, sizeof(double) * J, cudaMemcpyHostToDevice, c->stream));
+    // a shard writes only its own columns: start from the caller's values
+    FK_CUDA(c, cudaMemcpyAsync(d_out, out, sizeof(double) * (size_t)(m1 - m0), cudaMemcpyHostToDevice, c->stream));
+    w = d_w;
+  }
+  FK_CUDA(c, fk_launch_reduce(c->g, c->d_P[c->cur], w, m0, m1, d_partial,
+                              mem == FK_MEM_HOST ? d_out : out, c->stream));
+  c->launches += 2;
+  if (mem == FK_MEM_HOST) {
+    FK_CUDA(c, cudaMemcpyAsync(out, d_out, sizeof(double) * (size_t)(m1 - m0), cudaMemcpyDeviceToHost, c->stream));
+    FK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
+  }
   return FK_OK;
 }
 

@@ -169,6 +169,19 @@ __device__ __forceinline__ double contract_row(const FkGrid& g, const double2* _
   return acc;
 }
 
+// R22: weighted harmonic mean a b / (wa b + wb a), wa + wb = 1 the normalised Fritsch-Carlson
+// weights attached to a and b (wa = wb = 1/2 is Eq. 15); 0 unless a and b have the same sign.
+__device__ __forceinline__ double harmonic_w(double a, double b, double2 w) {
+  const double p = a * b;
+  const double r = rcp_newton(fma(w.x, b, w.y * a));
+  return p > 0.0 ? p * r : 0.0;
+}
+
+// global output-time column of lane `lane` of the context's local chunk `chunk` (column sharding)
+__device__ __forceinline__ int column_of(const FkGrid& g, int chunk, int lane) {
+  return (chunk * g.shard_count + g.shard_index) * FK_CW + lane;
+}
+
 // ---- mbarrier / TMA bulk-copy primitives (sm_90+ PTX; SASS: SYNCS.*, UBLKCP)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);

@@ -152,7 +152,7 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
   const int rows = min(T1, n1 - s1);                      // rows of this strip
   const uint32_t rec_bytes = (uint32_t)rows * sizeof(FkRec2);
   const uint32_t ubytes = u_line_bytes<T1>(g, s1);
-  const int m = chunk * FK_CW + lane;
+  const int m = fkd::column_of(g, chunk, lane);
   const bool active = m >= n && m <= N;
 
   if (leader) {

@@ -36,6 +36,12 @@ struct FkGrid {
   double inv_h0[3];       // (n-1)/(hi-lo)
   double dt, sq;          // sq = sqrt(2 dt)
   int validate;           // FK_FLAG_VALIDATE: report NaN / Inf coefficients of updated nodes
+  int periodic[3];        // dimension k is FK_FACE_PERIODIC (R21)
+  int weighted;           // FK_FLAG_WEIGHTED_SLOPES (R22)
+  int general_slopes;     // any periodic dimension or weighted slopes: fk_slopes takes its general path
+  int shard_index, shard_count;   // this context owns the chunks c with c % count == index
+  const double2* wgt[3];  // device, weighted only: per node the normalised weights (omega_a, omega_b)
+                          // attached to the two divided differences its slope is the mean of
   const double* x[3];     // device: node coordinates
   const double* inv_h[3]; // device: 1/(x[i+1]-x[i]), n-1 values
   double gh_a[3][FK_QMAX];
@@ -107,6 +113,11 @@ cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, 
 cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* Pold,
                                  const double* dP, double* Pnew, int n_chunks, int chunk0,
                                  int chunk1, int n, int N, cudaStream_t s);
+// out[m - m0] = sum_j w[j] P(t_m, x_j) for the owned columns m0 <= m < m1; partial: scratch of
+// FK_RED_BLOCKS * 32 doubles per chunk touched
+#define FK_RED_BLOCKS 64
+cudaError_t fk_launch_reduce(const FkGrid& g, const double* P, const double* w, int m0, int m1,
+                             double* partial, double* out, cudaStream_t s);
 cudaError_t fk_launch_gather_columns(const FkGrid& g, const double* P, int m0, int m1,
                                      double* out, cudaStream_t s);
 

@@ -117,7 +117,14 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
     for (int q = 0; q < g.Q[k]; ++q) {
       double z = fkd::push_point(centre, spread, g.gh_a[k][q]);
       const double w = g.gh_w[k][q];
-      if (z < lo) {
+      if (g.periodic[k]) {                       // R21: wrap into [lo, hi)
+        if (z < lo || z >= hi) {
+          const double L = hi - lo;
+          double r = fmod(z - lo, L);
+          if (r < 0.0) r += L;
+          z = lo + r;
+        }
+      } else if (z < lo) {
         if (g.face_kind[k][0] == 1) z = lo; else { ek += w * g.face_value[k][0]; continue; }
       } else if (z > hi) {
         if (g.face_kind[k][1] == 1) z = hi; else { ek += w * g.face_value[k][1]; continue; }
@@ -224,6 +231,53 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
 // ------------------------------------------------------------------------------------------
 constexpr int SR = 8;
 
+// The three nodes (a, b, c) whose two divided differences give the slope at node i of a line of
+// n nodes, and the cells ca (between a and b) and cb (between b and c): the node and its
+// neighbours inside; the first / last three nodes at the ends (R6); across the seam when the
+// dimension is periodic (R21: node n-1 is the image of node 0).
+struct SlopeWindow { int a, b, c, ca, cb; };
+__device__ __forceinline__ SlopeWindow slope_window(int i, int n, int periodic) {
+  SlopeWindow w;
+  if (periodic) {
+    w.b = i;
+    w.a = i == 0 ? n - 2 : i - 1;
+    w.c = i == n - 1 ? 1 : i + 1;
+    w.ca = i == 0 ? n - 2 : i - 1;
+    w.cb = i == n - 1 ? 0 : i;
+  } else {
+    const int la = min(max(i - 1, 0), n - 3);
+    w.a = la; w.b = la + 1; w.c = la + 2; w.ca = la; w.cb = la + 1;
+  }
+  return w;
+}
+
+// General slopes of one run (periodic dimensions and / or the weighted mean of R22): node by
+// node, three loads per dimension.  The streamlined code in fk_slopes covers everything else.
+template <int D>
+__device__ __forceinline__ void slopes_general(const FkGrid& g, const double* __restrict__ u,
+                                               double* __restrict__ o, size_t field, int line,
+                                               int i0) {
+  const int nl = g.n[D - 1];
+  int idx[3] = {0, 0, 0};
+  if (D == 2) idx[0] = line;
+  if (D == 3) { idx[0] = line / g.n[1]; idx[1] = line - idx[0] * g.n[1]; }
+  for (int q = 0; q < SR; ++q) {
+    const int i = i0 + q;
+    if (i >= nl) break;
+    idx[D - 1] = i;
+    const double* __restrict__ un = u + i * FK_CW;
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+      const int s = (int)g.stride[k] * FK_CW;
+      const SlopeWindow w = slope_window(idx[k], g.n[k], g.periodic[k]);
+      const double va = un[(w.a - idx[k]) * s], vb = un[(w.b - idx[k]) * s], vc = un[(w.c - idx[k]) * s];
+      const double da = (vb - va) * g.inv_h[k][w.ca], db = (vc - vb) * g.inv_h[k][w.cb];
+      o[(size_t)k * field + i * FK_CW] = g.weighted ? fkd::harmonic_w(da, db, g.wgt[k][idx[k]])
+                                                    : harmonic(da, db);
+    }
+  }
+}
+
 template <int D>
 __global__ void __launch_bounds__(256)
 fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP, int n_chunks,
@@ -241,6 +295,10 @@ fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP, int n
   double* __restrict__ o = dP + (size_t)c * chunk_elems + (size_t)node0 * FK_CW + threadIdx.x;
   const size_t field = (size_t)n_chunks * chunk_elems;
 
+  if (g.general_slopes) {                       // periodic dimensions and / or weighted means
+    slopes_general<D>(g, u, o, field, line, i0);
+    return;
+  }
   // values of the line at nodes i0-2 .. i0+SR (clamped; clamped duplicates are never selected)
   double v[SR + 3];
 #pragma unroll
@@ -305,7 +363,7 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   if (j >= jn) return;
   j += j0;
   const int c = chunk0 + blockIdx.y;
-  const int m = c * FK_CW + threadIdx.x;
+  const int m = fkd::column_of(g, c, threadIdx.x);
   const size_t chunk_elems = (size_t)g.J * FK_CW;
   const double* __restrict__ u = Pold + (size_t)c * chunk_elems + threadIdx.x;
   const double* __restrict__ d0 = dP + (size_t)c * chunk_elems + threadIdx.x;
@@ -326,7 +384,9 @@ fk_apply(FkGrid g, FkOperator op, const double* __restrict__ Pold,
 __global__ void fk_gather(FkGrid g, const double* __restrict__ P, int m0, int m1,
                           double* __restrict__ out) {
   __shared__ double tile[32][33];
-  const int c = m0 / FK_CW + blockIdx.y;
+  const int cg = m0 / FK_CW + blockIdx.y;                 // global chunk
+  if (cg % g.shard_count != g.shard_index) return;        // not this shard's: `out` is left alone
+  const int c = cg / g.shard_count;                        // local chunk
   const long long j0 = (long long)blockIdx.x * 32;
   for (int r = threadIdx.y; r < 32; r += blockDim.y) {
     long long j = j0 + r;
@@ -334,10 +394,48 @@ __global__ void fk_gather(FkGrid g, const double* __restrict__ P, int m0, int m1
   }
   __syncthreads();
   for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-    const int m = c * FK_CW + r;
+    const int m = cg * FK_CW + r;
     long long j = j0 + threadIdx.x;
     if (m >= m0 && m < m1 && j < g.J) out[(size_t)(m - m0) * g.J + j] = tile[threadIdx.x][r];
   }
+}
+
+// ------------------------------------------------------------------------------------------
+// fk_reduce_partial / fk_reduce_final: out[m - m0] = sum_j w_j P(t_m, x_j)
+// in two passes with a fixed summation order.  Pass 1: grid (FK_RED_BLOCKS, chunks touched),
+// block (32, 8): warp y of block b sums the nodes j = (b*8 + y) + k * (8*FK_RED_BLOCKS),
+// k = 0, 1, ...; the 8 warps are combined in order.  Pass 2: one warp per chunk adds the
+// FK_RED_BLOCKS partial sums in order.
+// ------------------------------------------------------------------------------------------
+__global__ void fk_reduce_partial(FkGrid g, const double* __restrict__ P,
+                                  const double* __restrict__ w, int chunk_first,
+                                  double* __restrict__ partial) {
+  __shared__ double sm[8][32];
+  const int cg = chunk_first + blockIdx.y;
+  if (cg % g.shard_count != g.shard_index) return;
+  const int c = cg / g.shard_count;
+  const double* __restrict__ Pc = P + (size_t)c * g.J * FK_CW + threadIdx.x;
+  double acc = 0.0;
+  for (long long j = (long long)blockIdx.x * 8 + threadIdx.y; j < g.J; j += 8LL * FK_RED_BLOCKS)
+    acc = fma(w[j], Pc[j * FK_CW], acc);
+  sm[threadIdx.y][threadIdx.x] = acc;
+  __syncthreads();
+  if (threadIdx.y == 0) {
+    double s = 0.0;
+    for (int y = 0; y < 8; ++y) s += sm[y][threadIdx.x];
+    partial[((size_t)blockIdx.y * FK_RED_BLOCKS + blockIdx.x) * FK_CW + threadIdx.x] = s;
+  }
+}
+
+__global__ void fk_reduce_final(FkGrid g, const double* __restrict__ partial, int chunk_first,
+                                int m0, int m1, double* __restrict__ out) {
+  const int cg = chunk_first + blockIdx.x;
+  if (cg % g.shard_count != g.shard_index) return;
+  const int m = cg * FK_CW + threadIdx.x;
+  double s = 0.0;
+  for (int b = 0; b < FK_RED_BLOCKS; ++b)
+    s += partial[((size_t)blockIdx.x * FK_RED_BLOCKS + b) * FK_CW + threadIdx.x];
+  if (m >= m0 && m < m1) out[m - m0] = s;
 }
 
 }  // namespace
@@ -388,6 +486,17 @@ cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, 
     fk_apply<2><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only, j0, jn);
   else
     fk_apply<3><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, n, N, far_only, j0, jn);
+  return cudaGetLastError();
+}
+
+cudaError_t fk_launch_reduce(const FkGrid& g, const double* P, const double* w, int m0, int m1,
+                             double* partial, double* out, cudaStream_t s) {
+  const int c0 = m0 / FK_CW, c1 = (m1 - 1) / FK_CW + 1;
+  dim3 block(32, 8), grid(FK_RED_BLOCKS, (unsigned)(c1 - c0));
+  fk_reduce_partial<<<grid, block, 0, s>>>(g, P, w, c0, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  fk_reduce_final<<<(unsigned)(c1 - c0), 32, 0, s>>>(g, partial, c0, m0, m1, out);
   return cudaGetLastError();
 }
 

@@ -26,7 +26,6 @@ namespace {
 constexpr int RB = 4;                      // rows per warp
 constexpr int H2 = FK_H;                   // dimension-2 halo of the blocked path
 constexpr int NS = 2 * H2 + 1;             // slots per row along dimension 2
-constexpr int NU = RB + NS - 1;            // union nodes of a group
 constexpr int EMAX = 16;                   // entries per row in dimension 0 / 1 (blocked path)
 constexpr int WARPS = 4;                   // a block = the same dimension-2 group of 4 dimension-1 lines
 constexpr int MINB = 3;                    // blocks per SM the register budget is set for
@@ -161,7 +160,7 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
   }
   if (ref < 0) {                                        // only Dirichlet rows: the constants
     for (int chunk = cfirst; chunk < clast; ++chunk) {
-      const int m = chunk * FK_CW + lane;
+      const int m = fkd::column_of(g, chunk, lane);
       double* __restrict__ out = Pnew + (size_t)chunk * chunk_elems + (size_t)jb * FK_CW + lane;
       for (int r = 0; r < rows; ++r)
         if (m >= n && m <= N) out[r * FK_CW] = op.c[jb + r];
@@ -169,7 +168,7 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     return;
   }
   // every load of the stage is issued before anything is compared (one round of latency)
-  bool ok = cref.x <= EMAX && cref.y <= EMAX;
+  bool ok = cref.x <= EMAX && cref.y <= EMAX && !g.periodic[2];   // a wrapped run has no static slots
   {
     const int dim = lane >> 4, e = lane & (EMAX - 1);   // lanes 0..15: dimension 0, 16..31: 1
     const int ne_ref = dim ? cref.y : cref.x;
@@ -243,7 +242,7 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
   }
   for (int chunk = cfirst; chunk < clast; ++chunk) {
-    const int m = chunk * FK_CW + lane;
+    const int m = fkd::column_of(g, chunk, lane);
     const bool active = m >= n && m <= N;
     const double* __restrict__ u = Pold + (size_t)chunk * chunk_elems + lane;
     const double* __restrict__ d0 = dP + (size_t)chunk * chunk_elems + lane;
