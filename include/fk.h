@@ -164,6 +164,26 @@ enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_FUSED = 3, FK_K_
 int fk_profile(fk_ctx* c, int on);
 int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
 
+/* Node-step updates each kernel class processed since the last fk_reset (rows it owns x active
+ * columns, Dirichlet rows excluded), host-side bookkeeping of fk_evolve: updates[FK_K_COUNT].
+ * FK_K_ASSEMBLE counts operator rows assembled (one per updated node and step). */
+int fk_profile_updates(fk_ctx* c, double* updates);
+
+/* Algorithmic work of the steps evolved since the last fk_reset, counted on the device while the
+ * operators are assembled (synchronises the stream): work[0] = node-step updates on rows the fused
+ * 2-D kernel owns, work[1] = their row-contraction multiply-adds, sum over steps of (active
+ * columns) x sum over rows of (d+1) prod_k D_k with D_k the distinct nodes the row touches along
+ * dimension k (the non-zeros of a row of Q Psi), work[2], work[3] = the same for
+ * all other updated rows.  The slopes of Eq. 15 cost about 14 d more operations per update
+ * (SURVEY.md section 8(d)). */
+int fk_work(fk_ctx* c, double work[4]);
+
+/* Measurement only, no context: the device's fp64 fused-multiply-add rate.  Launches
+ * 4 x (SM count) blocks x 512 threads, each thread running 8 independent chains of `iters`
+ * dependent fma; timed with CUDA events on `stream`, second of two launches.
+ * *tflops = 2 flops x 8 x iters x threads / time; *ms = that time. */
+int fk_peak_fp64(int device, void* stream, int iters, double* tflops, double* ms);
+
 /* Total kernels launched by this context since fk_create (all entry points). */
 long long fk_launch_count(const fk_ctx* c);
 

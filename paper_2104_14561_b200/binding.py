@@ -2,7 +2,8 @@
 
 Same names as the C entry points (`fk_create`, `fk_set_coeffs`, `fk_set_coeffs_range`,
 `fk_evolve`, `fk_reset`, `fk_read`, `fk_reduce`, `fk_check`, `fk_profile`, `fk_profile_read`,
-`fk_launch_count`, `fk_destroy`, `fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
+`fk_profile_updates`, `fk_work`, `fk_peak_fp64`, `fk_launch_count`, `fk_destroy`,
+`fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
 pointers) or torch CUDA tensors (device pointers); every step of the path runs in the CUDA
 kernels behind the ABI.  There is no CPU fallback: a missing library raises.
 """
@@ -26,7 +27,8 @@ KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock")
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 
 EXPORTS = ("fk_create", "fk_set_coeffs", "fk_set_coeffs_range", "fk_evolve", "fk_reset",
-           "fk_read", "fk_reduce", "fk_check", "fk_profile", "fk_profile_read", "fk_launch_count", "fk_destroy",
+           "fk_read", "fk_reduce", "fk_check", "fk_profile", "fk_profile_read",
+           "fk_profile_updates", "fk_work", "fk_peak_fp64", "fk_launch_count", "fk_destroy",
            "fk_last_error", "fk_gauss_hermite")
 
 
@@ -67,6 +69,9 @@ def lib():
         L.fk_check.argtypes = [vp]
         L.fk_profile.argtypes = [vp, C.c_int]
         L.fk_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+        L.fk_profile_updates.argtypes = [vp, dp]
+        L.fk_work.argtypes = [vp, dp]
+        L.fk_peak_fp64.argtypes = [C.c_int, vp, C.c_int, dp, dp]
         L.fk_launch_count.argtypes = [vp]
         L.fk_launch_count.restype = C.c_longlong
         L.fk_destroy.argtypes = [vp]
@@ -200,6 +205,29 @@ def fk_profile_read(ctx):
     ln = (C.c_longlong * FK_K_COUNT)()
     _check(ctx, lib().fk_profile_read(ctx, ms, ln))
     return {KERNEL_CLASSES[k]: (float(ms[k]), int(ln[k])) for k in range(FK_K_COUNT)}
+
+
+def fk_profile_updates(ctx):
+    """-> {class: node-step updates processed since the last fk_reset}."""
+    upd = (C.c_double * FK_K_COUNT)()
+    _check(ctx, lib().fk_profile_updates(ctx, upd))
+    return {KERNEL_CLASSES[k]: float(upd[k]) for k in range(FK_K_COUNT)}
+
+
+def fk_work(ctx):
+    """-> dict(updates_near, fma_near, updates_other, fma_other): algorithmic work counted on the device."""
+    w = (C.c_double * 4)()
+    _check(ctx, lib().fk_work(ctx, w))
+    return {"updates_near": w[0], "fma_near": w[1], "updates_other": w[2], "fma_other": w[3]}
+
+
+def fk_peak_fp64(device=0, stream=0, iters=1 << 15):
+    """-> (TFLOP/s, ms) of the DFMA microkernel (measurement only)."""
+    tf, ms = C.c_double(), C.c_double()
+    rc = lib().fk_peak_fp64(int(device), C.c_void_p(int(stream) or None), int(iters), C.byref(tf), C.byref(ms))
+    if rc != FK_OK:
+        raise FkError(rc, "fk_peak_fp64 failed")
+    return tf.value, ms.value
 
 
 def fk_launch_count(ctx):

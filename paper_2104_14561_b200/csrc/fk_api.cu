@@ -24,6 +24,7 @@ struct fk_ctx {
   FkGrid g;
   int N = 0, slots = 0, device = 0;
   int n_chunks = 0;                    // chunks this context owns (all of them unless sharded)
+  long long n_updated = 0;             // nodes that are not on an ABSORB face
   bool fused2d = false;                // 2-D: near rows go through fk_fused2d (else generic only)
   double2* d_wgt[3] = {nullptr, nullptr, nullptr};
   double* d_red = nullptr;             // fk_reduce: weights [J], partial sums, result
@@ -45,6 +46,8 @@ struct fk_ctx {
                       {nullptr, nullptr, nullptr, nullptr, nullptr}};
   cudaStream_t side = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_coef = nullptr;
+  unsigned long long* d_work = nullptr; // [N][4] per step: rows / sum prod D_k, near and other (fk_assemble)
+  double class_updates[FK_K_COUNT] = {0, 0, 0, 0, 0};   // node-step updates per kernel class
   int* d_status = nullptr;             // device status word: FK_BAD_* bits raised by fk_assemble
   int* h_status = nullptr;             // pinned host copy, refreshed at the end of every fk_evolve
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
@@ -165,6 +168,7 @@ void release(fk_ctx* c) {
   if (c->ev_coef) cudaEventDestroy(c->ev_coef);
   if (c->side) cudaStreamDestroy(c->side);
   cudaFree(c->d_far);
+  cudaFree(c->d_work);
   cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
   cudaFree(c->d_stage);
@@ -287,6 +291,9 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     gauss_hermite(p->Q[k], g.gh_a[k], g.gh_w[k]);
   }
   g.RS = qoff;
+  c->n_updated = 1;
+  for (int k = 0; k < p->d; ++k)
+    c->n_updated *= p->n[k] - (p->face_kind[k][0] == FK_FACE_ABSORB) - (p->face_kind[k][1] == FK_FACE_ABSORB);
 
 #define FK_CREATE_CUDA(call)                                                    \
   do {                                                                          \
@@ -362,6 +369,8 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_ready[i], cudaEventDisableTiming));
     FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_free[i], cudaEventDisableTiming));
   }
+  FK_CREATE_CUDA(cudaMalloc(&c->d_work, sizeof(unsigned long long) * 4 * (size_t)p->N));
+  FK_CREATE_CUDA(cudaMemsetAsync(c->d_work, 0, sizeof(unsigned long long) * 4 * (size_t)p->N, c->stream));
   FK_CREATE_CUDA(cudaMalloc(&c->d_status, sizeof(int)));
   FK_CREATE_CUDA(cudaMemsetAsync(c->d_status, 0, sizeof(int), c->stream));
   FK_CREATE_CUDA(cudaHostAlloc(&c->h_status, sizeof(int), cudaHostAllocDefault));
@@ -392,6 +401,8 @@ int fk_reset(fk_ctx* c) {
   FK_CUDA(c, fk_launch_fill_chi(c->g, c->d_P[1], c->n_chunks, c->stream));
   c->launches += 2;
   FK_CUDA(c, cudaMemsetAsync(c->d_status, 0, sizeof(int), c->stream));
+  FK_CUDA(c, cudaMemsetAsync(c->d_work, 0, sizeof(unsigned long long) * 4 * (size_t)c->N, c->stream));
+  for (int k = 0; k < FK_K_COUNT; ++k) c->class_updates[k] = 0.0;
   *c->h_status = 0;
   c->cur = 0;
   c->n_next = c->N;
@@ -517,12 +528,27 @@ int evolve_step(fk_ctx* c, int n) {
   cudaStream_t st = c->stream;
   FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
   FK_TRY(launch_on(c, c->side, FK_K_ASSEMBLE, "fk_assemble", [&] {
-    return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->side); }));
+    return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->d_work + 4 * (size_t)nu, c->side); }));
   FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
   FK_CUDA(c, cudaStreamWaitEvent(st, c->ev_ready[ob], 0));
   const bool fused = c->fused2d;
   const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
   const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
+  {                                                    // bookkeeping for fk_profile_updates
+    double cols = 0.0;                                 // active columns this context owns
+    for (int l = chunk0; l < last_chunk; ++l) {
+      const int m_lo = (l * c->g.shard_count + c->g.shard_index) * FK_CW;
+      const int a = m_lo > n ? m_lo : n, e = m_lo + FK_CW - 1 < c->N ? m_lo + FK_CW - 1 : c->N;
+      if (e >= a) cols += e - a + 1;
+    }
+    const double far_rows = fused ? far[0] : 0.0;
+    c->class_updates[FK_K_ASSEMBLE] += (double)c->n_updated;
+    if (fused) c->class_updates[FK_K_FUSED] += ((double)c->n_updated - far_rows) * cols;
+    if (generic) {
+      c->class_updates[FK_K_SLOPES] += (fused ? (double)(far[4] - (FK_FAR_BIG - far[3])) * c->g.n[1] : (double)c->g.J) * cols;
+      c->class_updates[c->g.d == 3 ? FK_K_ROWBLOCK : FK_K_APPLY] += (fused ? far_rows : (double)c->n_updated) * cols;
+    }
+  }
   if (fused)
     FK_TRY(launch_on(c, st, FK_K_FUSED, "fk_fused2d", [&] {
       return fk_launch_fused2d(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, st); }));
@@ -686,6 +712,61 @@ int fk_reduce(fk_ctx* c, const double* weights, int m0, int m1, double* out, int
     if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
   }
   return FK_OK;
+}
+
+int fk_profile_updates(fk_ctx* c, double* updates) {
+  if (!c) return FK_EINVAL;
+  if (!updates) return fail(c, FK_EINVAL, "updates is NULL");
+  for (int k = 0; k < FK_K_COUNT; ++k) updates[k] = c->class_updates[k];
+  return FK_OK;
+}
+
+int fk_work(fk_ctx* c, double work[4]) {
+  if (!c) return FK_EINVAL;
+  if (!work) return fail(c, FK_EINVAL, "work is NULL");
+  DeviceGuard guard(c->device);
+  std::vector<unsigned long long> h((size_t)4 * c->N);
+  FK_CUDA(c, cudaMemcpyAsync(h.data(), c->d_work, sizeof(unsigned long long) * h.size(), cudaMemcpyDeviceToHost, c->stream));
+  FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < 4; ++k) work[k] = 0.0;
+  for (int nu = 0; nu < c->N; ++nu) {                  // operator nu acts on the columns nu+1 .. N
+    const double cols = c->N - nu;
+    work[0] += (double)h[4 * (size_t)nu + 0] * cols;
+    work[1] += (double)h[4 * (size_t)nu + 1] * cols * (c->g.d + 1);
+    work[2] += (double)h[4 * (size_t)nu + 2] * cols;
+    work[3] += (double)h[4 * (size_t)nu + 3] * cols * (c->g.d + 1);
+  }
+  return FK_OK;
+}
+
+int fk_peak_fp64(int device, void* stream, int iters, double* tflops, double* ms) {
+  if (!tflops || !ms || iters < 1) return FK_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return FK_ECUDA;
+  DeviceGuard guard(device);
+  int sms = 0;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return FK_ECUDA;
+  const int blocks = 4 * sms, threads = 512;
+  cudaStream_t st = (cudaStream_t)stream;
+  double* out = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  int rc = FK_ECUDA;
+  float t = 0.f;
+  if (cudaMalloc(&out, sizeof(double) * (size_t)blocks * threads) != cudaSuccess) return FK_ENOMEM;
+  if (cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) == cudaSuccess &&
+      fk_launch_dfma_peak(out, blocks, threads, iters, st) == cudaSuccess &&      // warm-up
+      cudaEventRecord(e0, st) == cudaSuccess &&
+      fk_launch_dfma_peak(out, blocks, threads, iters, st) == cudaSuccess &&
+      cudaEventRecord(e1, st) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
+      cudaEventElapsedTime(&t, e0, e1) == cudaSuccess && t > 0.f) {
+    *ms = t;
+    *tflops = 2.0 * 8.0 * iters * (double)blocks * threads / (t * 1e-3) * 1e-12;
+    rc = FK_OK;
+  }
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(out);
+  return rc;
 }
 
 int fk_profile(fk_ctx* c, int on) {

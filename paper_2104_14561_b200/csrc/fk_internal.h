@@ -90,7 +90,10 @@ struct FkOperator {       // device pointers of one assembled A_nu
 // launchers (fk_kernels.cu); all asynchronous on `s`, return the launch's cudaError_t
 cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStream_t s);
 cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
-                               FkOperator op, int* status, cudaStream_t s);
+                               FkOperator op, int* status, unsigned long long* work,
+                               cudaStream_t s);
+// 2 x (iters x 8 chains) fused multiply-adds per thread on blocks x threads threads (fk_peak.cu)
+cudaError_t fk_launch_dfma_peak(double* out, int blocks, int threads, int iters, cudaStream_t s);
 // far_rows[slot] = number of rows of the step held in that coefficient slot that are not
 // FK_ROW_NEAR (2-D only), for the `count` steps step0.. whose slices sit at
 // coef + (step % slots) * 2*d*J (b then sigma); far_rows entries must be zeroed before

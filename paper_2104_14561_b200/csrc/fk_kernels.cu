@@ -48,11 +48,12 @@ __global__ void fk_fill_chi(FkGrid g, double* __restrict__ P, int n_chunks) {
 // its entries stay within FK_H nodes of the row's node: the weights of the 2*FK_H+1 nodes
 // around it per dimension, zero where no point lands.
 // ------------------------------------------------------------------------------------------
-__global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
-                            const double* __restrict__ sigma, FkOperator op,
-                            int* __restrict__ status) {
-  long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= g.J) return;
+// returns prod_k D_k of the row (-1 for a Dirichlet row); *is_near: the row has a compact record
+__device__ __forceinline__ int assemble_row(const FkGrid& g, const double* __restrict__ b,
+                                                 const double* __restrict__ sigma,
+                                                 const FkOperator& op, int* __restrict__ status,
+                                                 long long j, bool* is_near) {
+  *is_near = false;
   int idx[3];
   unravel(g, j, idx);
   int* cnt = op.cnt + j * 4;
@@ -71,7 +72,7 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
       for (int k = 0; k < 2; ++k)
         for (int e = 0; e < FK_NW; ++e) rec->w[k][e] = make_double2(0.0, 0.0);
     }
-    return;
+    return -1;
   }
   double2* __restrict__ roww = op.w + (size_t)j * g.RS;
   int* __restrict__ rowo = op.off + (size_t)j * g.RS;
@@ -172,6 +173,29 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
   if (rec) {
     rec->c = cj;
     rec->flags = near ? FK_ROW_NEAR : 0;
+  }
+  *is_near = near;
+  int prod = 1;
+  for (int k = 0; k < g.d; ++k) prod *= cnt[k];
+  return prod;
+}
+
+// work[0..3] += {updated rows with a compact record, their sum of prod_k D_k, the other updated
+// rows, their sum of prod_k D_k}: the algorithmic size of A_nu (one set of atomics per warp)
+__global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
+                            const double* __restrict__ sigma, FkOperator op,
+                            int* __restrict__ status, unsigned long long* __restrict__ work) {
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool near = false;
+  const int prod = j < g.J ? assemble_row(g, b, sigma, op, status, j, &near) : -1;
+  const bool live = prod >= 0;                            // an updated (non-Dirichlet) row
+  const unsigned near_rows = __reduce_add_sync(0xffffffffu, (live && near) ? 1u : 0u);
+  const unsigned far_rows = __reduce_add_sync(0xffffffffu, (live && !near) ? 1u : 0u);
+  const unsigned near_nnz = __reduce_add_sync(0xffffffffu, (live && near) ? (unsigned)prod : 0u);
+  const unsigned far_nnz = __reduce_add_sync(0xffffffffu, (live && !near) ? (unsigned)prod : 0u);
+  if ((threadIdx.x & 31) == 0) {
+    if (near_rows) { atomicAdd(work, (unsigned long long)near_rows); atomicAdd(work + 1, (unsigned long long)near_nnz); }
+    if (far_rows) { atomicAdd(work + 2, (unsigned long long)far_rows); atomicAdd(work + 3, (unsigned long long)far_nnz); }
   }
 }
 
@@ -454,8 +478,9 @@ cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStr
 }
 
 cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
-                               FkOperator op, int* status, cudaStream_t s) {
-  fk_assemble<<<node_blocks(g, 128), 128, 0, s>>>(g, b, sigma, op, status);
+                               FkOperator op, int* status, unsigned long long* work,
+                               cudaStream_t s) {
+  fk_assemble<<<node_blocks(g, 128), 128, 0, s>>>(g, b, sigma, op, status, work);
   return cudaGetLastError();
 }
 

@@ -22,7 +22,7 @@ def B():
 def declared_functions():
     text = open(os.path.join(ROOT, "include", "fk.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(fk_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(fk_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_declares_the_four_north_star_calls():
