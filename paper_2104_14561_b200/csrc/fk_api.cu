@@ -35,6 +35,8 @@ struct fk_ctx {
   double* d_coef = nullptr;            // [slots][2][d][J]: b then sigma per slot
   std::vector<int> slot_step;          // step held by each slot, -2 = empty
   bool autonomous = false;
+  bool auto_assembled = false;         // autonomous: A is the same every step and sits in op[0]
+  int auto_nu = 0;                     // ... assembled (and counted in d_work) under this step index
   double* d_P[2] = {nullptr, nullptr};  // both point FK_GUARD_ROWS rows into their allocations
   void* raw_P[2] = {nullptr, nullptr};
   void* raw_dP = nullptr;
@@ -404,6 +406,7 @@ int fk_reset(fk_ctx* c) {
   FK_CUDA(c, cudaMemsetAsync(c->d_work, 0, sizeof(unsigned long long) * 4 * (size_t)c->N, c->stream));
   for (int k = 0; k < FK_K_COUNT; ++k) c->class_updates[k] = 0.0;
   *c->h_status = 0;
+  c->auto_assembled = false;           // its work counters were just cleared: assemble once more
   c->cur = 0;
   c->n_next = c->N;
   for (auto& e : c->events) c->event_pool.push_back(e);
@@ -455,6 +458,7 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   FK_CUDA(c, cudaMemcpyAsync(c->d_coef + slice, sigma, sizeof(double) * slice, kind, c->stream));
   std::fill(c->slot_step.begin(), c->slot_step.end(), -2);
   c->autonomous = true;
+  c->auto_assembled = false;
   if (c->fused2d) {
     FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * FK_FAR_STRIDE, c->stream));
     FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, 0, 1, c->d_far, c->stream));
@@ -523,14 +527,19 @@ int evolve_step(fk_ctx* c, int n) {
   if (chunk0 >= last_chunk) return FK_OK;              // (sharded) none of this context's columns is active yet
   // assemble A_nu into buffer n & 1 on the side stream as soon as the kernels of step n + 2
   // (the buffer's previous users) are done; the kernels of this step wait for it
-  const int ob = n & 1;
+  // (an autonomous problem has one operator: assembled at the first step after a reset, reused)
+  const int ob = c->autonomous ? 0 : (n & 1);
   const FkOperator& op = c->op[ob];
   cudaStream_t st = c->stream;
-  FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
-  FK_TRY(launch_on(c, c->side, FK_K_ASSEMBLE, "fk_assemble", [&] {
-    return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->d_work + 4 * (size_t)nu, c->side); }));
-  FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
-  FK_CUDA(c, cudaStreamWaitEvent(st, c->ev_ready[ob], 0));
+  if (!(c->autonomous && c->auto_assembled)) {
+    FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
+    FK_TRY(launch_on(c, c->side, FK_K_ASSEMBLE, "fk_assemble", [&] {
+      return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->d_work + 4 * (size_t)nu, c->side); }));
+    FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
+    FK_CUDA(c, cudaStreamWaitEvent(st, c->ev_ready[ob], 0));
+    if (c->autonomous) { c->auto_assembled = true; c->auto_nu = nu; }
+    c->class_updates[FK_K_ASSEMBLE] += (double)c->n_updated;
+  }
   const bool fused = c->fused2d;
   const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
   const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
@@ -542,7 +551,6 @@ int evolve_step(fk_ctx* c, int n) {
       if (e >= a) cols += e - a + 1;
     }
     const double far_rows = fused ? far[0] : 0.0;
-    c->class_updates[FK_K_ASSEMBLE] += (double)c->n_updated;
     if (fused) c->class_updates[FK_K_FUSED] += ((double)c->n_updated - far_rows) * cols;
     if (generic) {
       c->class_updates[FK_K_SLOPES] += (fused ? (double)(far[4] - (FK_FAR_BIG - far[3])) * c->g.n[1] : (double)c->g.J) * cols;
@@ -574,7 +582,7 @@ int evolve_step(fk_ctx* c, int n) {
         return fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
                                fused ? 1 : 0, aj0, ajn, st); }));
   }
-  FK_CUDA(c, cudaEventRecord(c->ev_free[ob], st));
+  if (!c->autonomous) FK_CUDA(c, cudaEventRecord(c->ev_free[ob], st));
   return FK_OK;
 }
 
@@ -731,10 +739,12 @@ int fk_work(fk_ctx* c, double work[4]) {
   for (int k = 0; k < 4; ++k) work[k] = 0.0;
   for (int nu = 0; nu < c->N; ++nu) {                  // operator nu acts on the columns nu+1 .. N
     const double cols = c->N - nu;
-    work[0] += (double)h[4 * (size_t)nu + 0] * cols;
-    work[1] += (double)h[4 * (size_t)nu + 1] * cols * (c->g.d + 1);
-    work[2] += (double)h[4 * (size_t)nu + 2] * cols;
-    work[3] += (double)h[4 * (size_t)nu + 3] * cols * (c->g.d + 1);
+    // autonomous: one operator, counted where it was assembled, applied at every evolved step
+    const size_t at = 4 * (size_t)((c->autonomous && c->auto_assembled && nu >= c->n_next) ? c->auto_nu : nu);
+    work[0] += (double)h[at + 0] * cols;
+    work[1] += (double)h[at + 1] * cols * (c->g.d + 1);
+    work[2] += (double)h[at + 2] * cols;
+    work[3] += (double)h[at + 3] * cols * (c->g.d + 1);
   }
   return FK_OK;
 }

@@ -13,12 +13,21 @@
 // q = r + t, as in the fused 2-D kernel).  The kernel body is instantiated for the slot ranges
 // that occur (own node only -- where the dimension-2 motion vanishes a group reads 4 nodes --,
 // +-1, ..., all 2H+1), chosen per group by a warp-uniform test.
-// Groups whose rows disagree (a quadrature point of one row falls into the next cell), reach
-// beyond H nodes along dimension 2, or have more than EMAX entries in dimension 0 or 1, take the
-// row-at-a-time path (fkd::contract_row) inside the same kernel.
+// Groups whose rows disagree (a quadrature point of one row falls into the next cell) are
+// contracted on the union of the rows' entry lists (zero weights where a row has no entry);
+// groups that reach beyond H nodes along dimension 2 or need more than EMAX entries in
+// dimension 0 or 1 take the row-at-a-time path (fkd::contract_row) inside the same kernel.
+//
+// What bounds it (profiles/r2_rowblock3d_ncu_full.md): a node is 1 KB here (4 fields x 32
+// columns), so the L1 holds ~190 nodes and about half of the loads miss it; the L2 -> SM traffic
+// that results (~8 GB per chunk launch at ~4.5 TB/s) is the limiter, not DRAM, fp64 or issue.
+// One staging serves CPB = 2 chunks, and each group pulls its own rows of the plane L2PF steps
+// ahead into L2 with a bulk prefetch, so the misses are at least L2 hits.
 //
 // u and dP come from global memory through L1: a block is 4 warps = the same dimension-2 group of
 // 4 consecutive dimension-1 lines, whose dimension-0 / dimension-1 nodes largely coincide.
+#include <climits>
+
 #include "fk_device.cuh"
 
 namespace {
@@ -38,6 +47,9 @@ struct GroupStage {                        // per warp, shared memory
   double2 w2[RB][NS];
   int off0[EMAX], off1[EMAX];
   double c[RB];
+  int roff[2][RB][EMAX];                   // the rows' own lists, when they have to be merged
+  double2 rw[2][RB][EMAX];
+  int ucnt[2];
 };
 
 // The contraction of a group whose rows use only the dimension-2 slots TLO..THI: union nodes
@@ -168,11 +180,10 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     return;
   }
   // every load of the stage is issued before anything is compared (one round of latency)
-  bool ok = cref.x <= EMAX && cref.y <= EMAX && !g.periodic[2];   // a wrapped run has no static slots
+  bool ok = !g.periodic[2];                             // a wrapped run has no static slots
+  bool same = true;                                     // rows put their dimension-0 / 1 entries on the same nodes
   {
     const int dim = lane >> 4, e = lane & (EMAX - 1);   // lanes 0..15: dimension 0, 16..31: 1
-    const int ne_ref = dim ? cref.y : cref.x;
-    const bool mine = ok && e < ne_ref;
     const int q = g.qoff[dim] + e;
     const int q2 = g.qoff[2] + lane;
     int off01[RB], off2[RB];
@@ -182,27 +193,68 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     for (int r = 0; r < RB; ++r) {
       const bool dir = (cnt[r].w & FK_ROW_DIRICHLET) != 0;
       const size_t row = (size_t)(jb + r) * g.RS;
-      off01[r] = -1;
+      const int ne = dim ? cnt[r].y : cnt[r].x;
+      off01[r] = INT_MAX;                               // "no entry": sorts last in the merge
       off2[r] = 0;
       w01[r] = w2[r] = make_double2(0.0, 0.0);
-      if (!dir && mine) { off01[r] = op.off[row + q]; w01[r] = op.w[row + q]; }
+      ok = ok && cnt[r].x <= EMAX && cnt[r].y <= EMAX && cnt[r].z <= NS;
+      if (!dir && ne <= EMAX && e < ne) { off01[r] = op.off[row + q]; w01[r] = op.w[row + q]; }
       if (!dir && lane < cnt[r].z && lane < NS) { off2[r] = op.off[row + q2]; w2[r] = op.w[row + q2]; }
       if (lane == r && r < rows) cr = op.c[jb + r];
     }
-    int oref = -1;
+    int oref = INT_MAX;
 #pragma unroll
     for (int r = 0; r < RB; ++r) if (r == ref) oref = off01[r];
-    if (dim) st.off1[e] = oref; else st.off0[e] = oref;
     if (lane < RB * NS) st.w2[lane / NS][lane % NS] = make_double2(0.0, 0.0);
     if (lane < RB) st.c[lane] = cr;
+#pragma unroll
+    for (int r = 0; r < RB; ++r)
+      if (!(cnt[r].w & FK_ROW_DIRICHLET)) same = same && off01[r] == oref;
+    same = __all_sync(0xffffffffu, same);
+    ok = __all_sync(0xffffffffu, ok);
     __syncwarp();
+    if (same) {
+      if (dim) st.off1[e] = oref; else st.off0[e] = oref;
+#pragma unroll
+      for (int r = 0; r < RB; ++r)
+        if (dim) st.w1[r][e] = w01[r]; else st.w0[r][e] = w01[r];
+    } else if (ok) {
+      // the rows disagree somewhere (a quadrature point of one row fell into the next cell):
+      // contract them together on the UNION of their entry lists, zero weights where a row has no
+      // entry.  One lane per dimension merges the four ascending lists (rare path, <= 64 steps).
+#pragma unroll
+      for (int r = 0; r < RB; ++r) { st.roff[dim][r][e] = off01[r]; st.rw[dim][r][e] = w01[r]; }
+      __syncwarp();
+      if (e == 0) {
+        int head[RB] = {0, 0, 0, 0};
+        int k = 0;
+        for (;;) {
+          int lo = INT_MAX;
+#pragma unroll
+          for (int r = 0; r < RB; ++r)
+            if (head[r] < EMAX) lo = min(lo, st.roff[dim][r][head[r]]);
+          if (lo == INT_MAX) break;
+          if (k == EMAX) { k = EMAX + 1; break; }           // more than EMAX distinct nodes
+          if (dim) st.off1[k] = lo; else st.off0[k] = lo;
+#pragma unroll
+          for (int r = 0; r < RB; ++r) {
+            double2 w = make_double2(0.0, 0.0);
+            if (head[r] < EMAX && st.roff[dim][r][head[r]] == lo) w = st.rw[dim][r][head[r]++];
+            if (dim) st.w1[r][k] = w; else st.w0[r][k] = w;
+          }
+          ++k;
+        }
+        st.ucnt[dim] = k;
+      }
+      __syncwarp();
+      cref.x = st.ucnt[0];
+      cref.y = st.ucnt[1];
+      ok = cref.x <= EMAX && cref.y <= EMAX;
+    }
 #pragma unroll
     for (int r = 0; r < RB; ++r) {
-      const bool dir = (cnt[r].w & FK_ROW_DIRICHLET) != 0;
-      if (dim) st.w1[r][e] = w01[r]; else st.w0[r][e] = w01[r];
-      if (dir) continue;
-      ok = ok && cnt[r].x == cref.x && cnt[r].y == cref.y && cnt[r].z <= NS && off01[r] == oref;
-      if (lane < cnt[r].z && lane < NS) {
+      if (cnt[r].w & FK_ROW_DIRICHLET) continue;
+      if (ok && lane < cnt[r].z && lane < NS) {
         // dimension 2: entries -> slots around the row's own node (its stride is 1 node)
         const int t = off2[r] / FK_CW - (i2b + r) + H2;
         if (t >= 0 && t < NS) st.w2[r][t] = w2[r];
