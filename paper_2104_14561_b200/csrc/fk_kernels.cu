@@ -253,7 +253,7 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
 // two neighbours across lines.  End nodes use the first / last two divided differences (R6,
 // PAPER.md:160): with la = clamp(i-1, 0, n-3) the three nodes la, la+1, la+2 give both cases.
 // ------------------------------------------------------------------------------------------
-constexpr int SR = 8;
+constexpr int SR = 4;                 // nodes per warp; with 6 blocks per SM: measured best on config 5
 
 // The three nodes (a, b, c) whose two divided differences give the slope at node i of a line of
 // n nodes, and the cells ca (between a and b) and cb (between b and c): the node and its
@@ -303,7 +303,7 @@ __device__ __forceinline__ void slopes_general(const FkGrid& g, const double* __
 }
 
 template <int D>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 6)
 fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP, int n_chunks,
           int chunk0, int line0, int nlines) {
   const int nl = g.n[D - 1];
