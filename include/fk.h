@@ -155,12 +155,13 @@ int fk_check(fk_ctx* c);
 /* Per-kernel-class device time of the fk_evolve calls since the last fk_reset, measured with
  * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[FK_K_COUNT]
  * and launches[FK_K_COUNT] are indexed FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY (the generic
- * slopes / apply pair), FK_K_FUSED (the fused 2-D slopes+apply kernel) and FK_K_ROWBLOCK (the
- * 3-D apply kernel that contracts four rows at a time).  Synchronises the
+ * slopes / apply pair), FK_K_FUSED (the fused 2-D slopes+apply kernel), FK_K_ROWBLOCK (the
+ * 3-D apply kernel that contracts four rows at a time) and FK_K_FAR2D (the 2-D apply kernel of the
+ * rows the fused kernel leaves out).  Synchronises the
  * stream.  FK_K_ASSEMBLE is timed on the side stream, overlapped with other kernels: the classes
  * do not add up to the duration of the step. */
 enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_FUSED = 3, FK_K_ROWBLOCK = 4,
-       FK_K_COUNT = 5 };
+       FK_K_FAR2D = 5, FK_K_COUNT = 6 };
 int fk_profile(fk_ctx* c, int on);
 int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
 

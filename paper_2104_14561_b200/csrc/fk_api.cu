@@ -49,7 +49,7 @@ struct fk_ctx {
   cudaStream_t side = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_coef = nullptr;
   unsigned long long* d_work = nullptr; // [N][4] per step: rows / sum prod D_k, near and other (fk_assemble)
-  double class_updates[FK_K_COUNT] = {0, 0, 0, 0, 0};   // node-step updates per kernel class
+  double class_updates[FK_K_COUNT] = {0, 0, 0, 0, 0, 0};   // node-step updates per kernel class
   int* d_status = nullptr;             // device status word: FK_BAD_* bits raised by fk_assemble
   int* h_status = nullptr;             // pinned host copy, refreshed at the end of every fk_evolve
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
@@ -554,7 +554,7 @@ int evolve_step(fk_ctx* c, int n) {
     if (fused) c->class_updates[FK_K_FUSED] += ((double)c->n_updated - far_rows) * cols;
     if (generic) {
       c->class_updates[FK_K_SLOPES] += (fused ? (double)(far[4] - (FK_FAR_BIG - far[3])) * c->g.n[1] : (double)c->g.J) * cols;
-      c->class_updates[c->g.d == 3 ? FK_K_ROWBLOCK : FK_K_APPLY] += (fused ? far_rows : (double)c->n_updated) * cols;
+      c->class_updates[c->g.d == 3 ? FK_K_ROWBLOCK : fused ? FK_K_FAR2D : FK_K_APPLY] += (fused ? far_rows : (double)c->n_updated) * cols;
     }
   }
   if (fused)
@@ -562,12 +562,8 @@ int evolve_step(fk_ctx* c, int n) {
       return fk_launch_fused2d(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, st); }));
   if (generic) {
     // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
-    long long aj0 = 0, ajn = c->g.J;
     int sl0 = 0, sln = (int)(c->g.J / c->g.n[c->g.d - 1]);
     if (fused) {
-      const long long n1 = c->g.n[1];
-      aj0 = (long long)(FK_FAR_BIG - far[1]) * n1;
-      ajn = (long long)far[2] * n1 - aj0;
       sl0 = FK_FAR_BIG - far[3];
       sln = far[4] - sl0;
     }
@@ -577,10 +573,14 @@ int evolve_step(fk_ctx* c, int n) {
       FK_TRY(launch_on(c, st, FK_K_ROWBLOCK, "fk_rowblock3d", [&] {
         return fk_launch_rowblock3d(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n,
                                     c->N, st); }));
+    else if (fused)                                    // the rows the fused kernel left out
+      FK_TRY(launch_on(c, st, FK_K_FAR2D, "fk_far2d", [&] {
+        return fk_launch_far2d(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
+                               FK_FAR_BIG - far[1], far[2] - (FK_FAR_BIG - far[1]), st); }));
     else
       FK_TRY(launch_on(c, st, FK_K_APPLY, "fk_apply", [&] {
         return fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
-                               fused ? 1 : 0, aj0, ajn, st); }));
+                               0, 0, c->g.J, st); }));
   }
   if (!c->autonomous) FK_CUDA(c, cudaEventRecord(c->ev_free[ob], st));
   return FK_OK;

@@ -106,6 +106,45 @@ __device__ __forceinline__ void slopes_line(const FkGrid& g, const double* __res
   }
 }
 
+// The same for a line 1 <= l <= n0-2 of a strip whose slope window holds no first / last node of
+// dimension 1 and lies inside the grid with its +-1 neighbours: no clamps, no end rules, no
+// predicates -- straight-line code; ih[k] = 1/h of the cell right of node i_first-2+k is loop
+// invariant and lives in registers.
+template <int T1>
+struct SlopeRegs {
+  static constexpr int NPW = (Tile<T1>::W1 + Tile<T1>::NWARPS - 1) / Tile<T1>::NWARPS;
+  double ih[NPW + 3];
+};
+template <int T1>
+__device__ __forceinline__ void slopes_line_inner(const double* __restrict__ su,
+                                                  double* __restrict__ sd0,
+                                                  double* __restrict__ sd1,
+                                                  const SlopeRegs<T1>& sr, double iha, double ihb,
+                                                  int l, int warp, int lane) {
+  using T = Tile<T1>;
+  constexpr int NPW = SlopeRegs<T1>::NPW;
+  static_assert(NPW * T::NWARPS == T::W1, "every warp owns exactly NPW nodes of the slope window");
+  const int p0 = warp * NPW;
+  // u-window position of slope-window position p is p + 1
+  const double* __restrict__ ua = su + (((unsigned)(l - 1) % LBU) * T::WU + p0 + 1) * FK_CW + lane;
+  const double* __restrict__ ul = su + (((unsigned)l % LBU) * T::WU + p0 - 1) * FK_CW + lane;
+  const double* __restrict__ uc = su + (((unsigned)(l + 1) % LBU) * T::WU + p0 + 1) * FK_CW + lane;
+  double* __restrict__ o0 = sd0 + (((unsigned)l % LBD) * T::W1 + p0) * FK_CW + lane;
+  double* __restrict__ o1 = sd1 + (((unsigned)l % LBD) * T::W1 + p0) * FK_CW + lane;
+  double v[NPW + 2];                                // nodes i_first-1 .. i_first+NPW
+#pragma unroll
+  for (int k = 0; k < NPW + 2; ++k) v[k] = ul[(k + 1) * FK_CW];
+  double dl[NPW + 1];                               // dl[k]: cell right of node i_first-1+k
+#pragma unroll
+  for (int k = 0; k < NPW + 1; ++k) dl[k] = (v[k + 1] - v[k]) * sr.ih[k + 1];
+#pragma unroll
+  for (int k = 0; k < NPW; ++k) {
+    const double va = ua[k * FK_CW], vc = uc[k * FK_CW], vb = v[k + 1];
+    o0[k * FK_CW] = fkd::harmonic((vb - va) * iha, (vc - vb) * ihb);
+    o1[k * FK_CW] = fkd::harmonic(dl[k], dl[k + 1]);
+  }
+}
+
 // bytes and copies of one u line (nodes of the strip + halo + 1 that exist in the grid)
 template <int T1>
 __device__ __forceinline__ uint32_t u_line_bytes(const FkGrid& g, int s1) {
@@ -119,6 +158,52 @@ __device__ __forceinline__ void u_line_copy(const FkGrid& g, const double* __res
   const int a = max(0, s1 - H - 1);
   bulk_g2s(su + ((size_t)((unsigned)l % LBU) * T::WU + FK_UPOS(a)) * FK_CW,
            Pc + ((size_t)l * g.n[1] + a) * FK_CW, u_line_bytes<T1>(g, s1), bar);
+}
+
+// The lines t0 of a group's window that any of its RB rows uses, contracted with the rows'
+// dimension-1 weights restricted to the slots TLO..THI (union nodes q = TLO .. RB-1+THI); all
+// register indices are static.  Unused slots inside the range hold zero weights.
+template <int T1, int TLO, int THI>
+__device__ __forceinline__ void contract_lines(const double* __restrict__ su,
+                                               const double* __restrict__ sd0,
+                                               const FkRec2* __restrict__ rc,
+                                               const double2 (&w1)[RB][FK_NW], unsigned lines,
+                                               int i0, int ucol, int dcol, double (&acc)[RB]) {
+  using T = Tile<T1>;
+  int uslot = (unsigned)(i0 + LBU - H) % LBU, dslot = (unsigned)(i0 + LBD - H) % LBD;
+  for (int t0 = 0; t0 < FK_NW; ++t0) {
+    if ((lines >> t0) & 1u) {
+      const double* __restrict__ up = su + (uslot * (T::WU * FK_CW) + ucol);
+      const double* __restrict__ d0p = sd0 + (dslot * (T::W1 * FK_CW) + dcol);
+      const double* __restrict__ d1p = d0p + T::D_ELEMS;
+      double A[RB], A2[RB], B0[RB];
+#pragma unroll
+      for (int r = 0; r < RB; ++r) A[r] = A2[r] = B0[r] = 0.0;
+#pragma unroll
+      for (int q = TLO; q < RB + THI; ++q) {
+        // no per-node skipping: straight-line code lets the loads and the 3*RB
+        // accumulation chains of a line overlap
+        const double U = up[q * FK_CW], D0 = d0p[q * FK_CW], D1 = d1p[q * FK_CW];
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+          const int t = q - r;
+          if (t >= TLO && t <= THI) {
+            A[r] = fma(w1[r][t].x, U, A[r]);
+            A2[r] = fma(w1[r][t].y, D1, A2[r]);
+            B0[r] = fma(w1[r][t].x, D0, B0[r]);
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < RB; ++r) {
+        const double2 w0 = rc[r].w[0][t0];           // zero if row r does not use the line
+        acc[r] = fma(w0.x, A[r] + A2[r], acc[r]);
+        acc[r] = fma(w0.y, B0[r], acc[r]);
+      }
+    }
+    uslot = uslot + 1 == LBU ? 0 : uslot + 1;
+    dslot = dslot + 1 == LBD ? 0 : dslot + 1;
+  }
 }
 
 template <int T1>
@@ -154,6 +239,17 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
   const uint32_t ubytes = u_line_bytes<T1>(g, s1);
   const int m = fkd::column_of(g, chunk, lane);
   const bool active = m >= n && m <= N;
+
+  // A last strip that holds nothing but the nodes of an ABSORB face (n1 = k*T1 + 1, e.g. 129 or
+  // 257 nodes) has no row to contract: its rows are the constants g (R15), no window is needed.
+  if (rows == 1 && s1 == n1 - 1 && g.face_kind[1][1] == 0) {
+    if (active)
+      for (int i0 = L0 + (int)threadIdx.y; i0 < L1; i0 += 2 * T::NWARPS) {
+        const size_t j = (size_t)i0 * n1 + s1;
+        Pn[j * FK_CW + lane] = rec[j].c;
+      }
+    return;
+  }
 
   if (leader) {
     mbar_init(ubar, 1);
@@ -200,6 +296,12 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
     // ================= slope warps: per line i0, fetch u(i0+H+3) and rec(i0+1), then the
     // slopes of line i0+H+1 (needs u up to i0+H+2, fetched one iteration earlier)
     asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+    // strips whose slope window (nodes s1-H .. s1+T1+H-1) holds neither end node of dimension 1
+    // take the straight-line sweep on every line that is not the first / last of dimension 0
+    const bool inner1 = s1 - H >= 1 && s1 + T1 + H - 1 <= n1 - 2;
+    SlopeRegs<T1> sr;
+#pragma unroll
+    for (int k = 0; k < SlopeRegs<T1>::NPW + 3; ++k) sr.ih[k] = sih[warp * SlopeRegs<T1>::NPW + k];
     uint32_t uparity = 1;                                  // bit b: parity to wait for on ubar[b]
     for (int i0 = L0; i0 < L1; ++i0) {
       const bool more = i0 + 1 < L1;                       // a next line exists in this segment
@@ -228,7 +330,10 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
           bulk_g2s(srec + ((i0 + 1) & 1) * T1, rec + (size_t)(i0 + 1) * n1 + s1, rec_bytes, rb);
         }
       }
-      if (more && ld < n0) slopes_line<T1>(g, su, sd0, sd1, sih, iha, ihb, ld, s1, warp, lane);
+      if (more && ld < n0) {
+        if (inner1 && ld >= 1 && ld <= n0 - 2) slopes_line_inner<T1>(su, sd0, sd1, sr, iha, ihb, ld, warp, lane);
+        else slopes_line<T1>(g, su, sd0, sd1, sih, iha, ihb, ld, s1, warp, lane);
+      }
       asm volatile("bar.sync 1, %0;" ::"n"(T::THREADS) : "memory");
     }
     return;
@@ -255,7 +360,7 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
       double2 w1[RB][FK_NW];
       double acc[RB];
       unsigned m1[RB];
-      unsigned lines = 0, nodes = 0;
+      unsigned lines = 0;
       bool store[RB];
 #pragma unroll
       for (int r = 0; r < RB; ++r) {
@@ -265,7 +370,6 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
         store[r] = mine && active;
         m1[r] = mine ? (unsigned)rc[r].mask[1] : 0u;
         lines |= mine ? (unsigned)rc[r].mask[0] : 0u;
-        nodes |= m1[r] << r;
         acc[r] = valid ? rc[r].c : 0.0;
 #pragma unroll
         for (int t = 0; t < FK_NW; ++t) w1[r][t] = rc[r].w[1][t];
@@ -273,41 +377,14 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
       // the masks are the same in every lane; the reductions tell the compiler so (uniform
       // registers, plain branches instead of divergence bookkeeping)
       lines = __reduce_or_sync(0xffffffffu, lines);
-      nodes = __reduce_or_sync(0xffffffffu, nodes);
-      int uslot = (unsigned)(i0 + LBU - H) % LBU, dslot = (unsigned)(i0 + LBD - H) % LBD;
-      for (int t0 = 0; t0 < FK_NW; ++t0) {
-        if ((lines >> t0) & 1u) {
-          const double* __restrict__ up = su + (uslot * (T::WU * FK_CW) + ucol);
-          const double* __restrict__ d0p = sd0 + (dslot * (T::W1 * FK_CW) + dcol);
-          const double* __restrict__ d1p = d0p + T::D_ELEMS;
-          double A[RB], A2[RB], B0[RB];
-#pragma unroll
-          for (int r = 0; r < RB; ++r) A[r] = A2[r] = B0[r] = 0.0;
-#pragma unroll
-          for (int q = 0; q < RB + FK_NW - 1; ++q) {
-            // no per-node skipping: straight-line code lets the loads and the 3*RB
-            // accumulation chains of a line overlap; unused slots hold zero weights
-            const double U = up[q * FK_CW], D0 = d0p[q * FK_CW], D1 = d1p[q * FK_CW];
-#pragma unroll
-            for (int r = 0; r < RB; ++r) {
-              const int t = q - r;
-              if (t >= 0 && t < FK_NW) {
-                A[r] = fma(w1[r][t].x, U, A[r]);
-                A2[r] = fma(w1[r][t].y, D1, A2[r]);
-                B0[r] = fma(w1[r][t].x, D0, B0[r]);
-              }
-            }
-          }
-#pragma unroll
-          for (int r = 0; r < RB; ++r) {
-            const double2 w0 = rc[r].w[0][t0];           // zero if row r does not use the line
-            acc[r] = fma(w0.x, A[r] + A2[r], acc[r]);
-            acc[r] = fma(w0.y, B0[r], acc[r]);
-          }
-        }
-        uslot = uslot + 1 == LBU ? 0 : uslot + 1;
-        dslot = dslot + 1 == LBD ? 0 : dslot + 1;
-      }
+      // dimension-1 slots that carry a weight in any of the RB rows pick the variant of the sweep:
+      // a group whose points stay within +-1 node reads 6 union nodes per line instead of 8
+      unsigned slots = m1[0] | m1[1] | m1[2] | m1[3];
+      slots = __reduce_or_sync(0xffffffffu, slots);
+      if ((slots & ~0x0eu) == 0) contract_lines<T1, 1, 3>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
+      else if ((slots & ~0x0fu) == 0) contract_lines<T1, 0, 3>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
+      else if ((slots & ~0x1eu) == 0) contract_lines<T1, 1, 4>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
+      else contract_lines<T1, 0, 4>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
       double* __restrict__ out = Pn + ((size_t)i0 * n1 + s1 + warp * RB) * FK_CW + lane;
 #pragma unroll
       for (int r = 0; r < RB; ++r)

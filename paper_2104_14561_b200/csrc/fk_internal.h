@@ -112,6 +112,11 @@ cudaError_t fk_launch_slopes(const FkGrid& g, const double* P, double* dP, int n
 cudaError_t fk_launch_apply(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
                             double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
                             int far_only, long long j0, long long jn, cudaStream_t s);
+// 2-D apply of the rows that are not FK_ROW_NEAR on the lines line0 .. line0+nlines-1, four rows
+// adjacent along dimension 1 per warp (fk_far2d.cu); near and Dirichlet rows are left to fk_fused2d
+cudaError_t fk_launch_far2d(const FkGrid& g, FkOperator op, const double* Pold, const double* dP,
+                            double* Pnew, int n_chunks, int chunk0, int chunk1, int n, int N,
+                            int line0, int nlines, cudaStream_t s);
 // 3-D apply, four rows adjacent along dimension 2 per warp (fk_rowblock3d.cu); all rows
 cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* Pold,
                                  const double* dP, double* Pnew, int n_chunks, int chunk0,

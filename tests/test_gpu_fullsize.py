@@ -98,7 +98,7 @@ def test_config4_full_grid_prefix_and_deep_column(fk, oracle_mod):
     report("cfg4 401x201 prefix 8", got, ref)
     # the real near / far mix: the fused kernel and the far-row kernels all ran
     assert prof["fused"][1] == 8, prof
-    assert prof["apply"][1] + prof.get("far2d", (0.0, 0))[1] >= 8, prof
+    assert prof["far2d"][1] == 8 and prof["slopes"][1] == 8, prof
     m = 312
     wl = prefix_config(4, m)
     ref = oracle_mod.Oracle(wl).column_streamed(m)
