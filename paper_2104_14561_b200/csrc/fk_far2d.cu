@@ -90,9 +90,14 @@ fk_far2d(FkGrid g, FkOperator op, const double* __restrict__ Pold, const double*
     if (mine[r]) {
       if (ref < 0) { ref = r; n0e = cnt[r].x; }
       if (cnt[r].y > 0) {
-        const int* __restrict__ o = op.off + (size_t)(jb + r) * g.RS + q1;
-        qlo = min(qlo, o[0] / FK_CW);
-        qhi = max(qhi, o[cnt[r].y - 1] / FK_CW);
+        if (cnt[r].z) {                        // packed by fk_assemble: 1 + first node | last node << 16
+          qlo = min(qlo, (cnt[r].z & 0xffff) - 1);
+          qhi = max(qhi, cnt[r].z >> 16);
+        } else {
+          const int* __restrict__ o = op.off + (size_t)(jb + r) * g.RS + q1;
+          qlo = min(qlo, o[0] / FK_CW);
+          qhi = max(qhi, o[cnt[r].y - 1] / FK_CW);
+        }
         sum_d1 += cnt[r].y;
       }
     }

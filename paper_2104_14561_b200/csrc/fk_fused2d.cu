@@ -167,9 +167,16 @@ template <int T1, int TLO, int THI>
 __device__ __forceinline__ void contract_lines(const double* __restrict__ su,
                                                const double* __restrict__ sd0,
                                                const FkRec2* __restrict__ rc,
-                                               const double2 (&w1)[RB][FK_NW], unsigned lines,
+                                               const double2 (&wc)[RB][3], unsigned lines,
                                                int i0, int ucol, int dcol, double (&acc)[RB]) {
   using T = Tile<T1>;
+  // the centre slots 1..3 were fetched with the row heads (every variant needs them, and their
+  // latency overlaps the mask reduction); the outer slots only where the variant has them
+  double2 w1[RB][THI - TLO + 1];
+#pragma unroll
+  for (int r = 0; r < RB; ++r)
+#pragma unroll
+    for (int t = TLO; t <= THI; ++t) w1[r][t - TLO] = (t >= 1 && t <= 3) ? wc[r][t - 1] : rc[r].w[1][t];
   int uslot = (unsigned)(i0 + LBU - H) % LBU, dslot = (unsigned)(i0 + LBD - H) % LBD;
   for (int t0 = 0; t0 < FK_NW; ++t0) {
     if ((lines >> t0) & 1u) {
@@ -188,9 +195,9 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ su,
         for (int r = 0; r < RB; ++r) {
           const int t = q - r;
           if (t >= TLO && t <= THI) {
-            A[r] = fma(w1[r][t].x, U, A[r]);
-            A2[r] = fma(w1[r][t].y, D1, A2[r]);
-            B0[r] = fma(w1[r][t].x, D0, B0[r]);
+            A[r] = fma(w1[r][t - TLO].x, U, A[r]);
+            A2[r] = fma(w1[r][t - TLO].y, D1, A2[r]);
+            B0[r] = fma(w1[r][t - TLO].x, D0, B0[r]);
           }
         }
       }
@@ -357,22 +364,25 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
     // register indices are static: slot t of row r is union node q = r + t.
     {
       const FkRec2* __restrict__ rc = srec + (i0 & 1) * T1 + warp * RB;
-      double2 w1[RB][FK_NW];
       double acc[RB];
+      double2 wc[RB][3];
       unsigned m1[RB];
       unsigned lines = 0;
       bool store[RB];
 #pragma unroll
       for (int r = 0; r < RB; ++r) {
         const bool valid = warp * RB + r < rows;
-        const int flags = valid ? rc[r].flags : 0;
+        // c, flags and both masks of the row in one 16-byte load (FkRec2: c, then the flag word
+        // with mask[0] in bits 8-15 and mask[1] in bits 16-23)
+        const int4 head = *reinterpret_cast<const int4*>(&rc[r]);
+        const int flags = valid ? head.z : 0;
         const bool mine = (flags & (FK_ROW_NEAR | FK_ROW_DIRICHLET)) != 0;
         store[r] = mine && active;
-        m1[r] = mine ? (unsigned)rc[r].mask[1] : 0u;
-        lines |= mine ? (unsigned)rc[r].mask[0] : 0u;
-        acc[r] = valid ? rc[r].c : 0.0;
+        m1[r] = mine ? ((unsigned)flags >> 16) & 0xffu : 0u;
+        lines |= mine ? ((unsigned)flags >> 8) & 0xffu : 0u;
+        acc[r] = valid ? __hiloint2double(head.y, head.x) : 0.0;
 #pragma unroll
-        for (int t = 0; t < FK_NW; ++t) w1[r][t] = rc[r].w[1][t];
+        for (int t = 0; t < 3; ++t) wc[r][t] = rc[r].w[1][t + 1];
       }
       // the masks are the same in every lane; the reductions tell the compiler so (uniform
       // registers, plain branches instead of divergence bookkeeping)
@@ -381,10 +391,10 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
       // a group whose points stay within +-1 node reads 6 union nodes per line instead of 8
       unsigned slots = m1[0] | m1[1] | m1[2] | m1[3];
       slots = __reduce_or_sync(0xffffffffu, slots);
-      if ((slots & ~0x0eu) == 0) contract_lines<T1, 1, 3>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
-      else if ((slots & ~0x0fu) == 0) contract_lines<T1, 0, 3>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
-      else if ((slots & ~0x1eu) == 0) contract_lines<T1, 1, 4>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
-      else contract_lines<T1, 0, 4>(su, sd0, rc, w1, lines, i0, ucol, dcol, acc);
+      if ((slots & ~0x0eu) == 0) contract_lines<T1, 1, 3>(su, sd0, rc, wc, lines, i0, ucol, dcol, acc);
+      else if ((slots & ~0x0fu) == 0) contract_lines<T1, 0, 3>(su, sd0, rc, wc, lines, i0, ucol, dcol, acc);
+      else if ((slots & ~0x1eu) == 0) contract_lines<T1, 1, 4>(su, sd0, rc, wc, lines, i0, ucol, dcol, acc);
+      else contract_lines<T1, 0, 4>(su, sd0, rc, wc, lines, i0, ucol, dcol, acc);
       double* __restrict__ out = Pn + ((size_t)i0 * n1 + s1 + warp * RB) * FK_CW + lane;
 #pragma unroll
       for (int r = 0; r < RB; ++r)

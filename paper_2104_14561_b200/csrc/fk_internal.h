@@ -73,7 +73,7 @@ struct FkGrid {
 // slot t received an entry.  192 bytes, 16-byte aligned, so a line of records is one bulk copy.
 struct FkRec2 {
   double c;               // absorbed constant (= g on Dirichlet nodes)
-  int flags;              // FK_ROW_*
+  int flags;              // FK_ROW_* in bits 0-7, mask[0] in bits 8-15, mask[1] in bits 16-23
   int mask[2];            // used slots per dimension (0 on Dirichlet rows)
   int pad[3];
   double2 w[2][FK_NW];

@@ -168,11 +168,18 @@ __device__ __forceinline__ int assemble_row(const FkGrid& g, const double* __res
   }
   if (bad) atomicOr(status, bad);
   for (int k = g.d; k < 3; ++k) cnt[k] = 0;
+  // 2-D: first and last dimension-1 node of the row, packed into the unused third count (1 + first
+  // in the low half, last in the high half; 0 = not recorded), so that fk_far2d knows a group's
+  // union window from the counts alone
+  if (g.d == 2 && cnt[1] > 0 && g.n[1] < 65535)
+    cnt[2] = (1 + rowo[g.qoff[1]] / FK_CW) | ((rowo[g.qoff[1] + cnt[1] - 1] / FK_CW) << 16);
   cnt[3] = near ? FK_ROW_NEAR : 0;
   op.c[j] = cj;
   if (rec) {
     rec->c = cj;
-    rec->flags = near ? FK_ROW_NEAR : 0;
+    // the masks ride in the flag word (bits 8-15 / 16-23): the fused kernel fetches c, flags and
+    // masks of a row with one 16-byte load
+    rec->flags = (near ? FK_ROW_NEAR : 0) | (rec->mask[0] << 8) | (rec->mask[1] << 16);
   }
   *is_near = near;
   int prod = 1;
