@@ -330,6 +330,41 @@ fk_slopes(FkGrid g, const double* __restrict__ P, double* __restrict__ dP, int n
     slopes_general<D>(g, u, o, field, line, i0);
     return;
   }
+  // A run whose nodes and their +-1 neighbours are all inside the grid in every dimension (no
+  // first / last node of any line: no end rule, no clamp) takes straight-line code.
+  {
+    bool inner = i0 >= 1 && i0 + SR <= nl - 1;
+    int idx[2] = {0, 0};
+    if (D == 2) idx[0] = line;
+    if (D == 3) { idx[0] = line / g.n[1]; idx[1] = line - idx[0] * g.n[1]; }
+#pragma unroll
+    for (int k = 0; k < D - 1; ++k) inner = inner && idx[k] >= 1 && idx[k] <= g.n[k] - 2;
+    if (inner) {
+      double w[SR + 2];                                          // nodes i0-1 .. i0+SR
+#pragma unroll
+      for (int k = 0; k < SR + 2; ++k) w[k] = u[(i0 - 1 + k) * FK_CW];
+      const double* __restrict__ ih = g.inv_h[D - 1] + (i0 - 1);
+      double dl[SR + 1];                                         // dl[k]: cell right of node i0-1+k
+#pragma unroll
+      for (int k = 0; k < SR + 1; ++k) dl[k] = (w[k + 1] - w[k]) * ih[k];
+      double* __restrict__ ok = o + (size_t)(D - 1) * field + i0 * FK_CW;
+#pragma unroll
+      for (int k = 0; k < SR; ++k) ok[k * FK_CW] = harmonic(dl[k], dl[k + 1]);
+#pragma unroll
+      for (int k = 0; k < D - 1; ++k) {
+        const int s = (int)g.stride[k] * FK_CW;
+        const double iha = g.inv_h[k][idx[k] - 1], ihb = g.inv_h[k][idx[k]];
+        const double* __restrict__ un = u + i0 * FK_CW;
+        double* __restrict__ okk = o + (size_t)k * field + i0 * FK_CW;
+#pragma unroll
+        for (int q = 0; q < SR; ++q) {
+          const double va = un[q * FK_CW - s], vc = un[q * FK_CW + s], vb = w[q + 1];
+          okk[q * FK_CW] = harmonic((vb - va) * iha, (vc - vb) * ihb);
+        }
+      }
+      return;
+    }
+  }
   // values of the line at nodes i0-2 .. i0+SR (clamped; clamped duplicates are never selected)
   double v[SR + 3];
 #pragma unroll
