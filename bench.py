@@ -58,6 +58,29 @@ RING_SLOTS = 32                # coefficient ring for tables that are streamed (
 # name the commands).  An entry counts only while the kernel's source file is byte-identical to
 # the one profiled (sha1 below); otherwise `traffic` is null rather than stale.
 TRAFFIC = {
+    ("cfg4_runaway_2d", "far2d"): {
+        "source": "fk_far2d.cu", "source_sha1": "bb01a21dbabd7b31c53ace01530a2919c010bbed",
+        "dram_bytes": 404993280, "algorithmic_bytes": 171165120,
+        "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, 17.8e3 far rows); this path also "
+                  "reads the two slope fields: 32 B per update",
+        "profile": "profiles/r2_cfg4_kernels_ncu_full.md"},
+    ("cfg4_runaway_2d", "fused"): {
+        "source": "fk_fused2d.cu", "source_sha1": "5f85def52d3a1e844f8b3ff519b6858cee9757a0",
+        "dram_bytes": 795970816, "algorithmic_bytes": 600038400,
+        "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, 62.4e3 near rows; the kernel "
+                  "streams the whole grid)",
+        "profile": "profiles/r2_cfg4_kernels_ncu_full.md"},
+    ("cfg3_cellular_2d", "fused"): {
+        "source": "fk_fused2d.cu", "source_sha1": "5f85def52d3a1e844f8b3ff519b6858cee9757a0",
+        "dram_bytes": 310384896, "algorithmic_bytes": 311414160,
+        "launch": "step n = 424 of config 3's grid (601 active columns, 20 chunks)",
+        "profile": "profiles/r2_fused2d_ncu_full.md"},
+    ("cfg5_runaway_3d", "rowblock"): {
+        "source": "fk_rowblock3d.cu", "source_sha1": "98010baca72a85b8a6fb9372aad5f19e4d15f9c2",
+        "dram_bytes": 5395440000, "algorithmic_bytes": 646216704,
+        "launch": "step n = 48 of config 5's grid (49 active columns in 3 chunks: half of the lanes idle; this "
+                  "path also reads three slope fields: 40 B per update, and the factored rows per chunk group)",
+        "profile": "profiles/r2_cfg5_kernels_ncu_full.md"},
 }
 
 
