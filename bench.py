@@ -323,6 +323,8 @@ def roofline_of(B, runner, prof, prof_step_ms, upd, work, peak_hbm, peak_src, fp
     u_dom = upd[dom]
     if dom == "fused":
         flops = 2.0 * work["fma_near"] + SLOPE_FLOPS_PER_DIM * d * work["updates_near"]
+    elif dom == "line1d":                             # 1-D rows are counted as "other" by fk_assemble
+        flops = 2.0 * work["fma_other"] + SLOPE_FLOPS_PER_DIM * d * work["updates_other"]
     elif dom == "slopes":
         flops = SLOPE_FLOPS_PER_DIM * d * u_dom
     else:                                             # apply / rowblock / far2d: the rows outside the fused kernel
@@ -338,7 +340,7 @@ def roofline_of(B, runner, prof, prof_step_ms, upd, work, peak_hbm, peak_src, fp
     total_flops = 2.0 * (work["fma_near"] + work["fma_other"]) + SLOPE_FLOPS_PER_DIM * d * total_upd
     return {
         "bound": "alu" if alu_bound else "hbm",
-        "kernel": {"fused": "fk_fused2d", "apply": f"fk_apply<{d}>", "rowblock": "fk_rowblock3d", "far2d": "fk_far2d",
+        "kernel": {"fused": "fk_fused2d", "apply": f"fk_apply<{d}>", "rowblock": "fk_rowblock3d", "far2d": "fk_far2d", "line1d": "fk_line1d",
                    "slopes": f"fk_slopes<{d}>"}[dom],
         "achieved": fp64_tfs if alu_bound else hbm_gbs,
         "peak": fp64_tf if alu_bound else peak_hbm,

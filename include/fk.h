@@ -57,6 +57,13 @@ enum {
   FK_FLAG_VALIDATE = 1,  /* check every coefficient read by an updated node for NaN / Inf on the
                             device while the operator is assembled (costs two compares per
                             value); a hit is reported like a negative sigma, see fk_check */
+  FK_FLAG_MULTISTEP = 4, /* 1-D problems (no periodic face, Eq. 15 as printed, a line that fits shared
+                            memory): run the steps of an fk_evolve call in batches -- one launch
+                            assembles the operators of up to a few hundred steps, one launch applies
+                            them with each group of columns resident in shared memory (several
+                            operators per pass over P: SURVEY.md section 8(f)'s temporal blocking).
+                            Same results up to summation order.  Off by default: measured faster
+                            only on short lines */
   FK_FLAG_WEIGHTED_SLOPES = 2  /* nodal slopes by the Fritsch-Carlson weighted harmonic mean
                             (ref [17]; R22) instead of Eq. 15 as printed:
                             (w1+w2)/(w1/d_{j-1} + w2/d_j), w1 = 2h_j + h_{j-1}, w2 = h_j + 2h_{j-1};
@@ -120,7 +127,8 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
 /* Algorithm 1's loop for n = n_from, n_from-1, ..., n_to+1: assemble the
  * operator nu = n-1 once and update columns n..N.  The first call after fk_create/fk_reset
  * must have n_from = N; later calls continue where the previous one stopped (n_from = its
- * n_to); after n_to = 0 all columns are final.  Kernels are queued on the stream and the call
+ * n_to); after n_to = 0 all columns are final.  With FK_FLAG_MULTISTEP a 1-D problem
+ * runs its steps in batches (see the flag).  Kernels are queued on the stream and the call
  * returns without waiting for them, with one exception: on 2-D grids the first fk_evolve after
  * a coefficient load synchronises the stream once to read back, per loaded step, which rows
  * leave the fused kernel's halo (a few integers), so that the kernels of each step can be
@@ -156,12 +164,13 @@ int fk_check(fk_ctx* c);
  * CUDA events on the launching stream when profiling is on (fk_profile(c, 1)); ms[FK_K_COUNT]
  * and launches[FK_K_COUNT] are indexed FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY (the generic
  * slopes / apply pair), FK_K_FUSED (the fused 2-D slopes+apply kernel), FK_K_ROWBLOCK (the
- * 3-D apply kernel that contracts four rows at a time) and FK_K_FAR2D (the 2-D apply kernel of the
- * rows the fused kernel leaves out).  Synchronises the
+ * 3-D apply kernel that contracts four rows at a time), FK_K_FAR2D (the 2-D apply kernel of the
+ * rows the fused kernel leaves out) and FK_K_LINE1D (the 1-D kernel that runs a batch of steps per
+ * launch; its batch assembly is booked under FK_K_ASSEMBLE).  Synchronises the
  * stream.  FK_K_ASSEMBLE is timed on the side stream, overlapped with other kernels: the classes
  * do not add up to the duration of the step. */
 enum { FK_K_ASSEMBLE = 0, FK_K_SLOPES = 1, FK_K_APPLY = 2, FK_K_FUSED = 3, FK_K_ROWBLOCK = 4,
-       FK_K_FAR2D = 5, FK_K_COUNT = 6 };
+       FK_K_FAR2D = 5, FK_K_LINE1D = 6, FK_K_COUNT = 7 };
 int fk_profile(fk_ctx* c, int on);
 int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
 

@@ -21,8 +21,9 @@ FK_ALL_STEPS = -1
 FK_MAX_Q = 32
 FK_FLAG_VALIDATE = 1
 FK_FLAG_WEIGHTED_SLOPES = 2
-FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_ROWBLOCK, FK_K_FAR2D, FK_K_COUNT = 0, 1, 2, 3, 4, 5, 6
-KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock", "far2d")
+FK_FLAG_MULTISTEP = 4
+FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_ROWBLOCK, FK_K_FAR2D, FK_K_LINE1D, FK_K_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
+KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock", "far2d", "line1d")
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 

@@ -12,7 +12,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 LIB_PATH = os.path.join(_HERE, "libfk_b200.so")
-SOURCES = [os.path.join(_HERE, "csrc", f) for f in ("fk_api.cu", "fk_kernels.cu", "fk_fused2d.cu", "fk_rowblock3d.cu", "fk_far2d.cu", "fk_peak.cu")]
+SOURCES = [os.path.join(_HERE, "csrc", f) for f in ("fk_api.cu", "fk_kernels.cu", "fk_fused2d.cu", "fk_rowblock3d.cu", "fk_far2d.cu", "fk_line1d.cu", "fk_peak.cu")]
 HEADERS = [os.path.join(_HERE, "csrc", "fk_internal.h"), os.path.join(_HERE, "csrc", "fk_device.cuh"), os.path.join(_ROOT, "include", "fk.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]

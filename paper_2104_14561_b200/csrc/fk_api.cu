@@ -26,6 +26,9 @@ struct fk_ctx {
   int n_chunks = 0;                    // chunks this context owns (all of them unless sharded)
   long long n_updated = 0;             // nodes that are not on an ABSORB face
   bool fused2d = false;                // 2-D: near rows go through fk_fused2d (else generic only)
+  int line1d_cg = 0;                   // 1-D: column-group width of the multi-step kernel, 0 = step by step
+  int batch_cap = 0;                   // ... operators its batch storage holds
+  FkOperator opb = {nullptr, nullptr, nullptr, nullptr, nullptr};   // ... the batch storage
   double2* d_wgt[3] = {nullptr, nullptr, nullptr};
   double* d_red = nullptr;             // fk_reduce: weights [J], partial sums, result
   size_t red_bytes = 0;
@@ -49,7 +52,7 @@ struct fk_ctx {
   cudaStream_t side = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_coef = nullptr;
   unsigned long long* d_work = nullptr; // [N][4] per step: rows / sum prod D_k, near and other (fk_assemble)
-  double class_updates[FK_K_COUNT] = {0, 0, 0, 0, 0, 0};   // node-step updates per kernel class
+  double class_updates[FK_K_COUNT] = {0, 0, 0, 0, 0, 0, 0};   // node-step updates per kernel class
   int* d_status = nullptr;             // device status word: FK_BAD_* bits raised by fk_assemble
   int* h_status = nullptr;             // pinned host copy, refreshed at the end of every fk_evolve
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
@@ -169,6 +172,10 @@ void release(fk_ctx* c) {
   }
   if (c->ev_coef) cudaEventDestroy(c->ev_coef);
   if (c->side) cudaStreamDestroy(c->side);
+  cudaFree(c->opb.w);
+  cudaFree(c->opb.off);
+  cudaFree(c->opb.cnt);
+  cudaFree(c->opb.c);
   cudaFree(c->d_far);
   cudaFree(c->d_work);
   cudaFree(c->d_status);
@@ -237,7 +244,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   if (cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, p->device) != cudaSuccess ||
       cc_major != 10)
     return fail(nullptr, FK_ECUDA, "device is not compute capability 10.x: the kernels are built for sm_100a only");
-  if (p->flags & ~(unsigned)(FK_FLAG_VALIDATE | FK_FLAG_WEIGHTED_SLOPES))
+  if (p->flags & ~(unsigned)(FK_FLAG_VALIDATE | FK_FLAG_WEIGHTED_SLOPES | FK_FLAG_MULTISTEP))
     return fail(nullptr, FK_EINVAL, "unknown bits in flags");
   const int shard_count = p->shard_count <= 0 ? 1 : p->shard_count;
   if (p->shard_index < 0 || p->shard_index >= shard_count)
@@ -387,6 +394,24 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots * FK_FAR_STRIDE, c->stream));
     FK_CREATE_CUDA(fk_fused2d_setup());
     c->h_far.assign((size_t)slots * FK_FAR_STRIDE, 0);
+  }
+  if (p->d == 1 && (p->flags & FK_FLAG_MULTISTEP)) {
+    // the multi-step 1-D kernel: needs three copies of a column group's line in shared memory
+    int smem_max = 0;
+    FK_CREATE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+    c->line1d_cg = fk_line1d_group(g, (size_t)smem_max);
+    if (c->line1d_cg) {
+      const size_t per_step = (size_t)J * g.RS * (sizeof(double2) + sizeof(int)) + (size_t)J * (4 * sizeof(int) + sizeof(double));
+      long long cap = (long long)(((size_t)256 << 20) / per_step);
+      if (cap < 1) cap = 1;
+      if (cap > slots) cap = slots;          // a batch never outruns the loaded coefficient slots
+      c->batch_cap = (int)cap;
+      FK_CREATE_CUDA(cudaMalloc(&c->opb.w, sizeof(double2) * (size_t)cap * J * g.RS));
+      FK_CREATE_CUDA(cudaMalloc(&c->opb.off, sizeof(int) * (size_t)cap * J * g.RS));
+      FK_CREATE_CUDA(cudaMalloc(&c->opb.cnt, sizeof(int) * (size_t)cap * J * 4));
+      FK_CREATE_CUDA(cudaMalloc(&c->opb.c, sizeof(double) * (size_t)cap * J));
+      FK_CREATE_CUDA(fk_line1d_setup(g, c->line1d_cg));
+    }
   }
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[0], c->n_chunks, c->stream));
   FK_CREATE_CUDA(fk_launch_fill_chi(g, c->d_P[1], c->n_chunks, c->stream));
@@ -586,6 +611,45 @@ int evolve_step(fk_ctx* c, int n) {
   return FK_OK;
 }
 
+// active columns this context owns at step n (bookkeeping for fk_profile_updates)
+double active_columns(const fk_ctx* c, int n) {
+  double cols = 0.0;
+  for (int l = 0; l < c->n_chunks; ++l) {
+    const int m_lo = (l * c->g.shard_count + c->g.shard_index) * FK_CW;
+    const int a = m_lo > n ? m_lo : n, e = m_lo + FK_CW - 1 < c->N ? m_lo + FK_CW - 1 : c->N;
+    if (e >= a) cols += e - a + 1;
+  }
+  return cols;
+}
+
+// 1-D: the steps n, n-1, ..., n-count+1 of Algorithm 1 in two launches -- their operators into the
+// batch storage, then fk_line1d with every column group resident in shared memory over all of them
+int evolve_batch1d(fk_ctx* c, int n, int count) {
+  cudaStream_t st = c->stream;
+  if (!c->autonomous)
+    for (int k = 0; k < count; ++k) {
+      const int nu = n - 1 - k;
+      if (c->slot_step[nu % c->slots] != nu) {
+        char msg[96];
+        std::snprintf(msg, sizeof msg, "coefficients of step %d are not loaded", nu);
+        return fail(c, FK_ESTATE, msg);
+      }
+    }
+  if (!(c->autonomous && c->auto_assembled)) {
+    const int na = c->autonomous ? 1 : count;
+    FK_TRY(launch_on(c, st, FK_K_ASSEMBLE, "fk_assemble_batch", [&] {
+      return fk_launch_assemble_batch(c->g, c->d_coef, c->slots, n - 1, na, c->autonomous ? 1 : 0, c->opb,
+                                      c->d_status, c->d_work, st); }));
+    if (c->autonomous) { c->auto_assembled = true; c->auto_nu = n - 1; }
+    c->class_updates[FK_K_ASSEMBLE] += (double)c->n_updated * na;
+  }
+  for (int k = 0; k < count; ++k) c->class_updates[FK_K_LINE1D] += (double)c->n_updated * active_columns(c, n - k);
+  FK_TRY(launch_on(c, st, FK_K_LINE1D, "fk_line1d", [&] {
+    return fk_launch_line1d(c->g, c->opb, c->line1d_cg, count, n, c->autonomous ? 1 : 0, c->d_P[c->cur],
+                            c->d_P[c->cur ^ 1], c->n_chunks, c->N, st); }));
+  return FK_OK;
+}
+
 // after a failure inside a step: make the caller's stream wait for whatever the side stream
 // still has queued, so that the two never run unordered past the failing call (best effort)
 void join_side(fk_ctx* c) {
@@ -611,6 +675,19 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   // the side stream must see the coefficient copies queued on the caller's stream so far
   FK_CUDA(c, cudaEventRecord(c->ev_coef, c->stream));
   FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_coef, 0));
+  if (c->line1d_cg) {                 // 1-D: batches of steps, both P buffers end up current
+    for (int n = n_from; n > n_to;) {
+      const int left = n - n_to;
+      const int count = c->autonomous ? left : (left < c->batch_cap ? left : c->batch_cap);
+      const int rc = evolve_batch1d(c, n, count);
+      if (rc != FK_OK) { c->n_next = n; return rc; }
+      n -= count;
+      c->n_next = n;
+    }
+    if (n_from > n_to)
+      FK_CUDA(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    return FK_OK;
+  }
   for (int n = n_from; n > n_to; --n) {
     const int rc = evolve_step(c, n);
     if (rc != FK_OK) {

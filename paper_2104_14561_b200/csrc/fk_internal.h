@@ -92,6 +92,20 @@ cudaError_t fk_launch_fill_chi(const FkGrid& g, double* P, int n_chunks, cudaStr
 cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* sigma,
                                FkOperator op, int* status, unsigned long long* work,
                                cudaStream_t s);
+// operators of the steps nu_hi, nu_hi-1, ..., nu_hi-count+1 into consecutive operator-sized pieces
+// of `op` (1-D multi-step path); work + 4*nu counts rows / non-zeros like fk_launch_assemble
+cudaError_t fk_launch_assemble_batch(const FkGrid& g, const double* coef, int slots, int nu_hi,
+                                     int count, int autonomous, FkOperator op, int* status,
+                                     unsigned long long* work, cudaStream_t s);
+// 1-D, many steps per launch (fk_line1d.cu): column groups of cg columns keep their line in shared
+// memory over the steps n = n_hi .. n_hi-nsteps+1, operators from the batch `op`; reads Pcur, writes
+// the final state of the touched columns to BOTH buffers
+size_t fk_line1d_smem(const FkGrid& g, int cg);
+int fk_line1d_group(const FkGrid& g, size_t smem_limit);
+cudaError_t fk_line1d_setup(const FkGrid& g, int cg);
+cudaError_t fk_launch_line1d(const FkGrid& g, FkOperator op, int cg, int nsteps, int n_hi,
+                             int autonomous, double* Pcur, double* Pother, int n_chunks, int N,
+                             cudaStream_t s);
 // 2 x (iters x 8 chains) fused multiply-adds per thread on blocks x threads threads (fk_peak.cu)
 cudaError_t fk_launch_dfma_peak(double* out, int blocks, int threads, int iters, cudaStream_t s);
 // far_rows[slot] = number of rows of the step held in that coefficient slot that are not

@@ -206,6 +206,35 @@ __global__ void fk_assemble(FkGrid g, const double* __restrict__ b,
   }
 }
 
+// fk_assemble_batch: the operators of `count` consecutive steps nu = nu_hi, nu_hi-1, ... in one
+// launch (grid.y walks the steps), operator s of the batch stored at `op` + s * (its size): what
+// fk_line1d consumes.  An autonomous problem has count = 1 and the one coefficient slice.
+__global__ void fk_assemble_batch(FkGrid g, const double* __restrict__ coef, int slots, int nu_hi,
+                                  int count, int autonomous, FkOperator op,
+                                  int* __restrict__ status, unsigned long long* __restrict__ work) {
+  const size_t slice = (size_t)g.d * g.J;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  for (int s = blockIdx.y; s < count; s += gridDim.y) {
+    const int nu = nu_hi - s;
+    const double* __restrict__ b = coef + (size_t)(autonomous ? 0 : nu % slots) * 2 * slice;
+    FkOperator o;
+    o.w = op.w + (size_t)s * g.J * g.RS;
+    o.off = op.off + (size_t)s * g.J * g.RS;
+    o.cnt = op.cnt + (size_t)s * g.J * 4;
+    o.c = op.c + (size_t)s * g.J;
+    o.rec = nullptr;
+    bool near = false;
+    const int prod = j < g.J ? assemble_row(g, b, b + slice, o, status, j, &near) : -1;
+    const bool live = prod >= 0;
+    const unsigned rows = __reduce_add_sync(0xffffffffu, live ? 1u : 0u);
+    const unsigned nnz = __reduce_add_sync(0xffffffffu, live ? (unsigned)prod : 0u);
+    if ((threadIdx.x & 31) == 0 && rows) {
+      atomicAdd(work + 4 * (size_t)nu + 2, (unsigned long long)rows);
+      atomicAdd(work + 4 * (size_t)nu + 3, (unsigned long long)nnz);
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // fk_classify (2-D): how many rows of each loaded step are not FK_ROW_NEAR, by the same
 // fkd::reach test fk_assemble applies.  grid = (node blocks, min(steps, 4096)).
@@ -523,6 +552,14 @@ cudaError_t fk_launch_assemble(const FkGrid& g, const double* b, const double* s
                                FkOperator op, int* status, unsigned long long* work,
                                cudaStream_t s) {
   fk_assemble<<<node_blocks(g, 128), 128, 0, s>>>(g, b, sigma, op, status, work);
+  return cudaGetLastError();
+}
+
+cudaError_t fk_launch_assemble_batch(const FkGrid& g, const double* coef, int slots, int nu_hi,
+                                     int count, int autonomous, FkOperator op, int* status,
+                                     unsigned long long* work, cudaStream_t s) {
+  dim3 grid(node_blocks(g, 128), (unsigned)(count < 1024 ? count : 1024));
+  fk_assemble_batch<<<grid, 128, 0, s>>>(g, coef, slots, nu_hi, count, autonomous, op, status, work);
   return cudaGetLastError();
 }
 

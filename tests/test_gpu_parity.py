@@ -48,6 +48,45 @@ def test_small_config_matches_oracle(fk, oracle_P, idx):
     assert np.array_equal(got[0], ref[0])
 
 
+@pytest.mark.parametrize("idx", [1, 2])
+def test_1d_stepwise_and_multistep_paths(fk, oracle_P, idx):
+    """1-D problems run through the generic slopes / apply kernels by default and through fk_line1d
+    (batches of steps per launch) with FK_FLAG_MULTISTEP; both against the oracle, each through the
+    kernels it claims, whole run and in pieces (a batch boundary inside a 32-column chunk)."""
+    B, solve = fk
+    wl, ref = oracle_P(idx)
+    slots = 1 if wl.autonomous else wl.N
+    for flags, want, other in ((B.FK_FLAG_MULTISTEP, "line1d", "apply"), (0, "apply", "line1d")):
+        ctx = solve.create_for(wl, slots, flags=flags)
+        try:
+            B.fk_profile(ctx, True)
+            if wl.autonomous:
+                b, s = wl.coeffs(0)
+                B.fk_set_coeffs(ctx, B.FK_ALL_STEPS, b, s)
+            else:
+                b, s = wl.coeff_table(0, wl.N)
+                B.fk_set_coeffs_range(ctx, 0, wl.N, b, s)
+            cut = wl.N - 5
+            B.fk_evolve(ctx, wl.N, cut)
+            B.fk_evolve(ctx, cut, 0)
+            got = np.empty((wl.N + 1, wl.J))
+            B.fk_read(ctx, 0, wl.N + 1, got)
+            prof = B.fk_profile_read(ctx)
+            assert prof[want][1] > 0 and prof[other][1] == 0, prof
+            assert np.abs(got - ref).max() <= TOL, (flags, float(np.abs(got - ref).max()))
+            upd = B.fk_profile_updates(ctx)
+            assert upd[want] == pytest.approx(wl.updates - (wl.J - _updated(wl)) * wl.N * (wl.N + 1) / 2)
+        finally:
+            B.fk_destroy(ctx)
+
+
+def _updated(wl):
+    n = 1
+    for k in range(wl.d):
+        n *= wl.n[k] - int(wl.face_kind[k][0] == 0) - int(wl.face_kind[k][1] == 0)
+    return n
+
+
 @pytest.mark.parametrize("idx,slots", [(2, 7), (3, 1), (5, 4)])
 def test_coefficient_ring_equals_full_table(fk, oracle_P, idx, slots):
     _, solve = fk
