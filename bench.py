@@ -53,6 +53,7 @@ BYTES_PER_UPDATE = 16          # read P_old + write P_new, fp64 (SURVEY.md secti
 SLOPE_FLOPS_PER_DIM = 14       # Eq. 15 per update and dimension
 DEFAULT_CONFIG = 4
 RING_SLOTS = 32                # coefficient ring for tables that are streamed (config 5)
+SM_CLOCK_HZ = 1.965e9          # clocks.max.sm of the B200 (the run's own clock record is in `clocks`)
 
 # DRAM traffic of the dominant kernel from this round's `ncu --set full` captures (profiles/*.md
 # name the commands).  An entry counts only while the kernel's source file is byte-identical to
@@ -335,6 +336,17 @@ def roofline_of(B, runner, prof, prof_step_ms, upd, work, peak_hbm, peak_src, fp
     t_hbm = BYTES_PER_UPDATE * u_dom / (peak_hbm * 1e9)
     t_fp64 = flops / (fp64_tf * 1e12)
     alu_bound = t_fp64 > t_hbm
+    # the operand roof of a contraction without register reuse: every
+    # multiply-add takes one 8-byte u / dP operand per lane through the 128 B/clk L1 / shared-memory
+    # data stage = 16 multiply-adds per clock and SM; context for the kernels whose rows share no nodes
+    operand = None
+    if dom in ("apply", "far2d", "rowblock", "line1d"):
+        contraction = 2.0 * work["fma_other"]
+        roof = 16.0 * sm_count * SM_CLOCK_HZ
+        operand = {"achieved_fma_per_s": contraction / 2.0 / secs, "roof_fma_per_s": roof,
+                   "frac": contraction / 2.0 / secs / roof,
+                   "note": "1 operand per multiply-add: 16 FMA/clk/SM x SMs x 1.965 GHz (128 B/clk data stage, "
+                           "B300_MICROARCH guide); row-blocked paths (banded far rows, 3-D groups) may exceed it"}
     tr = traffic_for(wl.name, dom)
     total_upd = work["updates_near"] + work["updates_other"]
     total_flops = 2.0 * (work["fma_near"] + work["fma_other"]) + SLOPE_FLOPS_PER_DIM * d * total_upd
@@ -353,6 +365,7 @@ def roofline_of(B, runner, prof, prof_step_ms, upd, work, peak_hbm, peak_src, fp
                  "peak_source": (f"fk_peak_fp64 in this process: {4 * sm_count} blocks x 512 threads x 8 chains x "
                                  f"{fp64_iters} dependent fma x 2 flops in {fp64_ms:.3f} ms (second launch, CUDA events)")},
         "floor_ms": {"hbm": t_hbm * 1e3, "fp64": t_fp64 * 1e3},
+        "operand_roof": operand,
         "traffic": tr["dram_bytes"] if tr else None,
         "traffic_note": (f"ncu dram bytes of the launch {tr['launch']}; algorithmic bytes of that launch: "
                          f"{tr['algorithmic_bytes']}; {tr['profile']}") if tr else
