@@ -57,6 +57,8 @@ struct fk_ctx {
   int* h_status = nullptr;             // pinned host copy, refreshed at the end of every fk_evolve
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
   std::vector<int> h_far;              // host copy, valid when far_valid
+  int* d_far_line = nullptr;           // [slots][n0] far rows per line of each loaded step
+  std::vector<int> h_far_line;         // host copy, valid when far_valid
   bool far_valid = false;
   int sm_count = 148;
   double* d_stage = nullptr;           // fk_read staging for host destinations
@@ -177,6 +179,7 @@ void release(fk_ctx* c) {
   cudaFree(c->opb.cnt);
   cudaFree(c->opb.c);
   cudaFree(c->d_far);
+  cudaFree(c->d_far_line);
   cudaFree(c->d_work);
   cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
@@ -275,6 +278,8 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   g.weighted = (p->flags & FK_FLAG_WEIGHTED_SLOPES) ? 1 : 0;
   g.shard_index = p->shard_index;
   g.shard_count = shard_count;
+  g.near_lo = 0;
+  g.near_hi = p->n[0];
   int qoff = 0;
   for (int k = 0; k < 3; ++k) { g.n[k] = 1; g.Q[k] = 0; g.stride[k] = 0; }
   long long st = 1;
@@ -394,6 +399,9 @@ int fk_create(const fk_params* p, fk_ctx** out) {
     FK_CREATE_CUDA(cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)slots * FK_FAR_STRIDE, c->stream));
     FK_CREATE_CUDA(fk_fused2d_setup());
     c->h_far.assign((size_t)slots * FK_FAR_STRIDE, 0);
+    FK_CREATE_CUDA(cudaMalloc(&c->d_far_line, sizeof(int) * (size_t)slots * p->n[0]));
+    FK_CREATE_CUDA(cudaMemsetAsync(c->d_far_line, 0, sizeof(int) * (size_t)slots * p->n[0], c->stream));
+    c->h_far_line.assign((size_t)slots * p->n[0], 0);
   }
   if (p->d == 1 && (p->flags & FK_FLAG_MULTISTEP)) {
     // the multi-step 1-D kernel: needs three copies of a column group's line in shared memory
@@ -463,7 +471,11 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
     FK_CUDA(c, cudaMemsetAsync(c->d_far + (size_t)s0 * FK_FAR_STRIDE, 0, sizeof(int) * (size_t)first * FK_FAR_STRIDE, c->stream));
     if (count > first)
       FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * (size_t)(count - first) * FK_FAR_STRIDE, c->stream));
-    FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, step0, count, c->d_far, c->stream));
+    const size_t n0 = (size_t)c->g.n[0];
+    FK_CUDA(c, cudaMemsetAsync(c->d_far_line + (size_t)s0 * n0, 0, sizeof(int) * (size_t)first * n0, c->stream));
+    if (count > first)
+      FK_CUDA(c, cudaMemsetAsync(c->d_far_line, 0, sizeof(int) * (size_t)(count - first) * n0, c->stream));
+    FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, step0, count, c->d_far, c->d_far_line, c->stream));
     ++c->launches;
     c->far_valid = false;
   }
@@ -486,7 +498,8 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   c->auto_assembled = false;
   if (c->fused2d) {
     FK_CUDA(c, cudaMemsetAsync(c->d_far, 0, sizeof(int) * FK_FAR_STRIDE, c->stream));
-    FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, 0, 1, c->d_far, c->stream));
+    FK_CUDA(c, cudaMemsetAsync(c->d_far_line, 0, sizeof(int) * (size_t)c->g.n[0], c->stream));
+    FK_CUDA(c, fk_launch_classify(c->g, c->d_coef, c->slots, 0, 1, c->d_far, c->d_far_line, c->stream));
     ++c->launches;
     c->far_valid = false;
   }
@@ -528,6 +541,53 @@ const char* status_text(int bits) {
   return "";
 }
 
+// 2-D: who takes which rows of one step.  The fused kernel costs the same per line whatever share
+// of the line's rows it owns, so the lines at either end of dimension 0 on which at least half of
+// the updated rows are far (config 4: p < ~12) are left to fk_far2d whole -- their near rows are
+// assembled without the FK_ROW_NEAR flag (FkGrid::near_lo / near_hi) -- and the fused kernel runs on
+// the output lines line_lo .. line_hi-1 only.  Lines of Dirichlet nodes need no kernel at all (both P
+// buffers hold chi there from the start).
+struct Plan2D {
+  int line_lo = 0, line_hi = 0;   // output lines of the fused kernel
+  double other_rows = 0.0;        // updated rows it leaves out (far rows + the near rows of skipped lines)
+  int fl0 = 0, fl1 = 0;           // lines holding such rows: fl0 .. fl1-1 (fk_far2d)
+  int sl0 = 0, sl1 = 0;           // lines their entries touch: sl0 .. sl1-1 (fk_slopes)
+};
+
+Plan2D plan_2d(const fk_ctx* c, int slot) {
+  const FkGrid& g = c->g;
+  const int n0 = g.n[0], n1 = g.n[1];
+  const int* far = &c->h_far[(size_t)slot * FK_FAR_STRIDE];
+  const int* fl = &c->h_far_line[(size_t)slot * n0];
+  const int upl = n1 - (g.face_kind[1][0] == FK_FACE_ABSORB) - (g.face_kind[1][1] == FK_FACE_ABSORB);
+  const int first = g.face_kind[0][0] == FK_FACE_ABSORB ? 1 : 0;          // updated lines: first .. last-1
+  const int last = g.face_kind[0][1] == FK_FACE_ABSORB ? n0 - 1 : n0;
+  Plan2D p;
+  int lo = first, hi = last;
+  while (lo < hi && 2 * fl[lo] >= upl) ++lo;
+  while (hi > lo && 2 * fl[hi - 1] >= upl) --hi;
+  p.line_lo = lo;
+  p.line_hi = hi;
+  p.other_rows = far[0];
+  p.fl0 = p.sl0 = n0;
+  if (far[0] > 0) {
+    p.fl0 = FK_FAR_BIG - far[1]; p.fl1 = far[2];
+    p.sl0 = FK_FAR_BIG - far[3]; p.sl1 = far[4];
+  }
+  auto hand_over = [&](int a, int b) {               // lines a .. b-1 go to fk_far2d whole
+    if (a >= b) return;
+    for (int l = a; l < b; ++l) p.other_rows += upl - fl[l];
+    p.fl0 = a < p.fl0 ? a : p.fl0;
+    p.fl1 = b > p.fl1 ? b : p.fl1;
+    const int s0 = a - FK_H > 0 ? a - FK_H : 0, s1 = b + FK_H < n0 ? b + FK_H : n0;   // near rows reach FK_H lines
+    p.sl0 = s0 < p.sl0 ? s0 : p.sl0;
+    p.sl1 = s1 > p.sl1 ? s1 : p.sl1;
+  };
+  hand_over(first, lo);
+  hand_over(hi, last);
+  return p;
+}
+
 // one step of Algorithm 1: assemble A_nu (nu = n-1) on the side stream,
 // update columns n..N on the caller's stream
 int evolve_step(fk_ctx* c, int n) {
@@ -556,18 +616,20 @@ int evolve_step(fk_ctx* c, int n) {
   const int ob = c->autonomous ? 0 : (n & 1);
   const FkOperator& op = c->op[ob];
   cudaStream_t st = c->stream;
+  const bool fused = c->fused2d;
+  const Plan2D plan = fused ? plan_2d(c, slot) : Plan2D();
   if (!(c->autonomous && c->auto_assembled)) {
+    FkGrid gs = c->g;                                  // this step's range of lines with FK_ROW_NEAR rows
+    if (fused) { gs.near_lo = plan.line_lo; gs.near_hi = plan.line_hi; }
     FK_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_free[ob], 0));
     FK_TRY(launch_on(c, c->side, FK_K_ASSEMBLE, "fk_assemble", [&] {
-      return fk_launch_assemble(c->g, b, b + slice, op, c->d_status, c->d_work + 4 * (size_t)nu, c->side); }));
+      return fk_launch_assemble(gs, b, b + slice, op, c->d_status, c->d_work + 4 * (size_t)nu, c->side); }));
     FK_CUDA(c, cudaEventRecord(c->ev_ready[ob], c->side));
     FK_CUDA(c, cudaStreamWaitEvent(st, c->ev_ready[ob], 0));
     if (c->autonomous) { c->auto_assembled = true; c->auto_nu = nu; }
     c->class_updates[FK_K_ASSEMBLE] += (double)c->n_updated;
   }
-  const bool fused = c->fused2d;
-  const int* far = fused ? &c->h_far[(size_t)slot * FK_FAR_STRIDE] : nullptr;
-  const bool generic = !fused || far[0] > 0;           // rows the fused kernel leaves out
+  const bool generic = !fused || plan.other_rows > 0;  // rows the fused kernel leaves out
   {                                                    // bookkeeping for fk_profile_updates
     double cols = 0.0;                                 // active columns this context owns
     for (int l = chunk0; l < last_chunk; ++l) {
@@ -575,22 +637,22 @@ int evolve_step(fk_ctx* c, int n) {
       const int a = m_lo > n ? m_lo : n, e = m_lo + FK_CW - 1 < c->N ? m_lo + FK_CW - 1 : c->N;
       if (e >= a) cols += e - a + 1;
     }
-    const double far_rows = fused ? far[0] : 0.0;
-    if (fused) c->class_updates[FK_K_FUSED] += ((double)c->n_updated - far_rows) * cols;
+    if (fused) c->class_updates[FK_K_FUSED] += ((double)c->n_updated - plan.other_rows) * cols;
     if (generic) {
-      c->class_updates[FK_K_SLOPES] += (fused ? (double)(far[4] - (FK_FAR_BIG - far[3])) * c->g.n[1] : (double)c->g.J) * cols;
-      c->class_updates[c->g.d == 3 ? FK_K_ROWBLOCK : fused ? FK_K_FAR2D : FK_K_APPLY] += (fused ? far_rows : (double)c->n_updated) * cols;
+      c->class_updates[FK_K_SLOPES] += (fused ? (double)(plan.sl1 - plan.sl0) * c->g.n[1] : (double)c->g.J) * cols;
+      c->class_updates[c->g.d == 3 ? FK_K_ROWBLOCK : fused ? FK_K_FAR2D : FK_K_APPLY] += (fused ? plan.other_rows : (double)c->n_updated) * cols;
     }
   }
-  if (fused)
+  if (fused && plan.line_hi > plan.line_lo)
     FK_TRY(launch_on(c, st, FK_K_FUSED, "fk_fused2d", [&] {
-      return fk_launch_fused2d(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, st); }));
+      return fk_launch_fused2d(c->g, op, Pold, Pnew, chunk0, last_chunk, n, c->N, c->sm_count, plan.line_lo,
+                               plan.line_hi, st); }));
   if (generic) {
-    // all nodes, or (2-D) only the lines that hold far rows / that their entries touch
+    // all nodes, or (2-D) only the lines that hold rows outside the fused kernel / that their entries touch
     int sl0 = 0, sln = (int)(c->g.J / c->g.n[c->g.d - 1]);
     if (fused) {
-      sl0 = FK_FAR_BIG - far[3];
-      sln = far[4] - sl0;
+      sl0 = plan.sl0;
+      sln = plan.sl1 - plan.sl0;
     }
     FK_TRY(launch_on(c, st, FK_K_SLOPES, "fk_slopes", [&] {
       return fk_launch_slopes(c->g, Pold, c->d_dP, c->n_chunks, chunk0, last_chunk, sl0, sln, st); }));
@@ -601,7 +663,7 @@ int evolve_step(fk_ctx* c, int n) {
     else if (fused)                                    // the rows the fused kernel left out
       FK_TRY(launch_on(c, st, FK_K_FAR2D, "fk_far2d", [&] {
         return fk_launch_far2d(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
-                               FK_FAR_BIG - far[1], far[2] - (FK_FAR_BIG - far[1]), st); }));
+                               plan.fl0, plan.fl1 - plan.fl0, st); }));
     else
       FK_TRY(launch_on(c, st, FK_K_APPLY, "fk_apply", [&] {
         return fk_launch_apply(c->g, op, Pold, c->d_dP, Pnew, c->n_chunks, chunk0, last_chunk, n, c->N,
@@ -668,6 +730,8 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
   DeviceGuard guard(c->device);
   if (c->fused2d && !c->far_valid && n_from > n_to) {  // one small read-back per coefficient load
     FK_CUDA(c, cudaMemcpyAsync(c->h_far.data(), c->d_far, sizeof(int) * (size_t)c->slots * FK_FAR_STRIDE,
+                               cudaMemcpyDeviceToHost, c->stream));
+    FK_CUDA(c, cudaMemcpyAsync(c->h_far_line.data(), c->d_far_line, sizeof(int) * c->h_far_line.size(),
                                cudaMemcpyDeviceToHost, c->stream));
     FK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->far_valid = true;

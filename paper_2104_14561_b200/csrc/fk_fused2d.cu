@@ -216,7 +216,8 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ su,
 template <int T1>
 __global__ void __launch_bounds__(Tile<T1>::THREADS, 2)
 fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ Pold,
-           double* __restrict__ Pnew, int chunk0, int n, int N, int nstrips, int seg_len) {
+           double* __restrict__ Pnew, int chunk0, int n, int N, int nstrips, int seg_len,
+           int line_lo, int line_hi) {
   using T = Tile<T1>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* su = reinterpret_cast<double*>(smem_raw);
@@ -236,7 +237,7 @@ fk_fused2d(FkGrid g, const FkRec2* __restrict__ rec, const double* __restrict__ 
   const int n0 = g.n[0], n1 = g.n[1];
   const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
   const int s1 = strip * T1;
-  const int L0 = seg * seg_len, L1 = min(n0, L0 + seg_len);
+  const int L0 = line_lo + seg * seg_len, L1 = min(line_hi, L0 + seg_len);   // output lines of this block
   const int chunk = chunk0 + blockIdx.y;
   const size_t chunk_elems = (size_t)g.J * FK_CW;
   const double* __restrict__ Pc = Pold + (size_t)chunk * chunk_elems;
@@ -413,22 +414,24 @@ cudaError_t fk_fused2d_setup(void) {
 }
 
 cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold, double* Pnew,
-                              int chunk0, int chunk1, int n, int N, int sm_count,
-                              cudaStream_t s) {
+                              int chunk0, int chunk1, int n, int N, int sm_count, int line_lo,
+                              int line_hi, cudaStream_t s) {
   constexpr int T1 = 16;
-  const int n0 = g.n[0], n1 = g.n[1];
+  const int n1 = g.n[1];
+  const int nl = line_hi - line_lo;                         // output lines line_lo .. line_hi-1
+  if (nl <= 0) return cudaSuccess;
   const int nstrips = (n1 + T1 - 1) / T1;
   const int nchunks = chunk1 - chunk0;
   // enough blocks for about six waves of two blocks per SM, segments of at least 16 lines
   const long long want = 6LL * 2 * sm_count;
   long long nseg = (want + (long long)nstrips * nchunks - 1) / ((long long)nstrips * nchunks);
-  const int max_seg = n0 / 16 > 1 ? n0 / 16 : 1;
+  const int max_seg = nl / 16 > 1 ? nl / 16 : 1;
   if (nseg > max_seg) nseg = max_seg;
   if (nseg < 1) nseg = 1;
-  const int seg_len = (int)((n0 + nseg - 1) / nseg);
-  nseg = (n0 + seg_len - 1) / seg_len;
+  const int seg_len = (int)((nl + nseg - 1) / nseg);
+  nseg = (nl + seg_len - 1) / seg_len;
   dim3 block(FK_CW, 2 * Tile<T1>::NWARPS), grid((unsigned)(nstrips * nseg), (unsigned)nchunks);
   fk_fused2d<T1><<<grid, block, Tile<T1>::SMEM, s>>>(g, op.rec, Pold, Pnew, chunk0, n, N,
-                                                      nstrips, seg_len);
+                                                      nstrips, seg_len, line_lo, line_hi);
   return cudaGetLastError();
 }

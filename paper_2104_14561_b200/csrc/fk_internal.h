@@ -40,6 +40,8 @@ struct FkGrid {
   int weighted;           // FK_FLAG_WEIGHTED_SLOPES (R22)
   int general_slopes;     // any periodic dimension or weighted slopes: fk_slopes takes its general path
   int shard_index, shard_count;   // this context owns the chunks c with c % count == index
+  int near_lo, near_hi;           // 2-D: only rows on the lines near_lo .. near_hi-1 may be FK_ROW_NEAR (set per
+                                  // step by fk_evolve: lines where most rows are far go to fk_far2d whole)
   const double2* wgt[3];  // device, weighted only: per node the normalised weights (omega_a, omega_b)
                           // attached to the two divided differences its slope is the mean of
   const double* x[3];     // device: node coordinates
@@ -111,13 +113,15 @@ cudaError_t fk_launch_dfma_peak(double* out, int blocks, int threads, int iters,
 // far_rows[slot] = number of rows of the step held in that coefficient slot that are not
 // FK_ROW_NEAR (2-D only), for the `count` steps step0.. whose slices sit at
 // coef + (step % slots) * 2*d*J (b then sigma); far_rows entries must be zeroed before
+// far_line[slot * n[0] + i0] = how many of them sit on line i0 (zeroed before, like far_rows)
 cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, int step0,
-                               int count, int* far_rows, cudaStream_t s);
+                               int count, int* far_rows, int* far_line, cudaStream_t s);
 // fused 2-D kernel: slopes + apply for the FK_ROW_NEAR and Dirichlet rows of every active
 // column; P never leaves the chip between the two (fk_fused2d.cu)
+// ... on the output lines line_lo .. line_hi-1 (rows elsewhere are not FK_ROW_NEAR, g.near_lo / near_hi)
 cudaError_t fk_launch_fused2d(const FkGrid& g, FkOperator op, const double* Pold, double* Pnew,
-                              int chunk0, int chunk1, int n, int N, int sm_count,
-                              cudaStream_t s);
+                              int chunk0, int chunk1, int n, int N, int sm_count, int line_lo,
+                              int line_hi, cudaStream_t s);
 cudaError_t fk_fused2d_setup(void);
 // slopes of the lines line0 .. line0+nlines-1 (a line = one run of the fastest dimension; J / n[d-1]
 // lines in all); apply on the nodes j0 .. j0+jn-1 only (jn = J: all nodes)

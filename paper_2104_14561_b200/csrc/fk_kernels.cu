@@ -94,7 +94,7 @@ __device__ __forceinline__ int assemble_row(const FkGrid& g, const double* __res
     if (rec) {
       int first, last;
       fkd::reach(g, k, centre, spread, &first, &last);
-      rec_k = first >= rbase && last <= idx[k] + FK_H;
+      rec_k = first >= rbase && last <= idx[k] + FK_H && idx[0] >= g.near_lo && idx[0] < g.near_hi;
       near = near && rec_k;
       if (rec_k)
         for (int e = 0; e < FK_NW; ++e) rec->w[k][e] = make_double2(0.0, 0.0);
@@ -240,7 +240,7 @@ __global__ void fk_assemble_batch(FkGrid g, const double* __restrict__ coef, int
 // fkd::reach test fk_assemble applies.  grid = (node blocks, min(steps, 4096)).
 // ------------------------------------------------------------------------------------------
 __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots, int step0,
-                            int count, int* __restrict__ far_rows) {
+                            int count, int* __restrict__ far_rows, int* __restrict__ far_line) {
   const size_t slice = (size_t)g.d * g.J;
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int idx[3] = {0, 0, 0};
@@ -263,6 +263,7 @@ __global__ void fk_classify(FkGrid g, const double* __restrict__ coef, int slots
       }
     }
     int* __restrict__ f = far_rows + slot * FK_FAR_STRIDE;
+    if (far) atomicAdd(far_line + (size_t)slot * g.n[0] + idx[0], 1);   // far rows per line
     const unsigned m = __ballot_sync(0xffffffffu, far);
     if (m) {                                  // one set of atomics per warp that holds far rows
       const int a1 = __reduce_max_sync(0xffffffffu, far ? FK_FAR_BIG - idx[0] : 0);
@@ -564,9 +565,9 @@ cudaError_t fk_launch_assemble_batch(const FkGrid& g, const double* coef, int sl
 }
 
 cudaError_t fk_launch_classify(const FkGrid& g, const double* coef, int slots, int step0,
-                               int count, int* far_rows, cudaStream_t s) {
+                               int count, int* far_rows, int* far_line, cudaStream_t s) {
   dim3 grid(node_blocks(g, 128), (unsigned)(count < 4096 ? count : 4096));
-  fk_classify<<<grid, 128, 0, s>>>(g, coef, slots, step0, count, far_rows);
+  fk_classify<<<grid, 128, 0, s>>>(g, coef, slots, step0, count, far_rows, far_line);
   return cudaGetLastError();
 }
 

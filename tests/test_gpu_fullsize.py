@@ -12,6 +12,7 @@ column before it), so deep columns and prefixes are compared exactly:
              kernel AND the far-row kernels (the real near / far mix at small p)
   config 5   161 x 81 x 65: prefix N' = 3 (one oracle application costs ~15 s of 4 cores; the
              64-step prefix SURVEY.md section 8(d) asks for would be ~9 hours)
+  FK_SLOW=1  config 3 m = 2000 (= N), config 4 m = 1250 (= N/4), config 5 prefix 6
 
 The worst error of each case is printed (run with -s to see it; recorded in DESIGN.md section 4).
 """
@@ -104,6 +105,21 @@ def test_config4_full_grid_prefix_and_deep_column(fk, oracle_mod):
     ref = oracle_mod.Oracle(wl).column_streamed(m)
     got, _ = gpu_columns(fk, wl, m, m + 1)
     report(f"cfg4 401x201 column {m}", got[0], ref)
+
+
+@pytest.mark.skipif(not os.environ.get("FK_SLOW"), reason="minutes of oracle time: FK_SLOW=1 (run once per round, profiles/r2_parity_fullsize.md)")
+def test_slow_deeper_cases(fk, oracle_mod):
+    """Deeper than the default suite affords: config 4 at m = 1250 (= N/4: 1250 nonlinear steps of
+    the real near / far mix) and config 5 for a 6-step prefix (21 oracle applications)."""
+    m = 1250
+    wl = prefix_config(4, m)
+    ref = oracle_mod.Oracle(wl).column_streamed(m)
+    got, _ = gpu_columns(fk, wl, m, m + 1)
+    report(f"cfg4 401x201 column {m}", got[0], ref)
+    wl = prefix_config(5, 6)
+    ref = oracle_mod.Oracle(wl).algorithm1()
+    got, _ = gpu_columns(fk, wl, 0, 7)
+    report("cfg5 161x81x65 prefix 6", got, ref)
 
 
 def test_config5_full_grid_prefix(fk, oracle_mod):
