@@ -61,19 +61,20 @@ SM_CLOCK_HZ = 1.965e9          # clocks.max.sm of the B200 (the run's own clock 
 TRAFFIC = {
     ("cfg4_runaway_2d", "far2d"): {
         "source": "fk_far2d.cu", "source_sha1": "bb01a21dbabd7b31c53ace01530a2919c010bbed",
-        "dram_bytes": 404993280, "algorithmic_bytes": 171165120,
-        "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, 17.8e3 far rows); this path also "
+        "dram_bytes": 450597632, "algorithmic_bytes": 193100000,
+        "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, about 20.1e3 rows: 17.8e3 far rows "
+                  "and the near rows of the lines handed over whole); this path also "
                   "reads the two slope fields: 32 B per update",
         "profile": "profiles/r2_cfg4_kernels_ncu_full.md"},
     ("cfg4_runaway_2d", "fused"): {
-        "source": "fk_fused2d.cu", "source_sha1": "5f85def52d3a1e844f8b3ff519b6858cee9757a0",
-        "dram_bytes": 795970816, "algorithmic_bytes": 600038400,
-        "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, 62.4e3 near rows; the kernel "
-                  "streams the whole grid)",
+        "source": "fk_fused2d.cu", "source_sha1": "a69b7c46b8f12346ea4808a2f39802e3470c1529",
+        "dram_bytes": 650159104, "algorithmic_bytes": 578100000,
+        "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, about 60.1e3 near rows on the "
+                  "output lines ~95..399; 39 idle lanes in the first chunk)",
         "profile": "profiles/r2_cfg4_kernels_ncu_full.md"},
     ("cfg3_cellular_2d", "fused"): {
-        "source": "fk_fused2d.cu", "source_sha1": "5f85def52d3a1e844f8b3ff519b6858cee9757a0",
-        "dram_bytes": 310384896, "algorithmic_bytes": 311414160,
+        "source": "fk_fused2d.cu", "source_sha1": "a69b7c46b8f12346ea4808a2f39802e3470c1529",
+        "dram_bytes": 308636928, "algorithmic_bytes": 311414160,
         "launch": "step n = 424 of config 3's grid (601 active columns, 20 chunks)",
         "profile": "profiles/r2_fused2d_ncu_full.md"},
     ("cfg5_runaway_3d", "rowblock"): {
