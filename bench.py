@@ -493,10 +493,13 @@ def run_cuda(args, wl, rank, world):
     # one evolution of each other configuration, same process (per_config)
     per_config = {}
     if rank == 0 and not args.no_per_config:
-        for idx in (1, 2, 3, 4, 5):
+        # BASELINE.json's configs 1-5 in full; the section 8(f) workloads 6 (the paper's periodic cellular
+        # flow, in full) and 7 (config 5 on the paper's radial grid with weighted slopes: its first 96
+        # steps, i.e. columns 0..96 of the full run -- a full evolution is 3.3e12 updates)
+        for idx in (1, 2, 3, 4, 5, 6, 7):
             if idx == args.config:
                 continue
-            w2 = W.config(idx)
+            w2 = W.config(idx) if idx != 7 else W.config(7, N=96, dt=W.config(7).dt)
             tb = (1 if w2.autonomous else w2.N) * 2 * w2.d * w2.J * 8
             res2 = tb < 40e9
             r2 = Runner(B, torch, w2, dev, stream, res2)
@@ -521,7 +524,7 @@ def run_cuda(args, wl, rank, world):
                 p2, pms2, u2, wk2 = profile_pass(B, torch, r2, not res2)
                 rl2 = roofline_of(B, r2, p2, pms2, u2, wk2, peak, peak_src, fp64_tf, fp64_ms, fp64_iters, sm_count)
                 per_config[w2.name] = {
-                    "grid": list(w2.n), "N": w2.N, "updates": w2.updates, "ms_per_evolution": ms2,
+                    "grid": list(w2.n), "N": w2.N, "prefix_of_N": W.config(7).N if idx == 7 else None, "updates": w2.updates, "ms_per_evolution": ms2,
                     "updates_per_s": w2.updates / (ms2 * 1e-3),
                     "coefficients": "resident in HBM" if res2 else f"streamed through a ring of {RING_SLOTS} slots "
                                     "(generated on the host and uploaded between the timed fk_evolve pieces)",
