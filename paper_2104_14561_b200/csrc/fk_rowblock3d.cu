@@ -40,6 +40,7 @@ constexpr int WARPS = 4;                   // a block = the same dimension-2 gro
 constexpr int MINB = 3;                    // blocks per SM the register budget is set for
 constexpr int CPB = 2;                     // chunks served by one staging of a group's rows
 constexpr int L2PF = 3;                    // planes ahead whose rows a group pulls into L2
+constexpr int WMAX2 = 32;                  // widest dimension-2 union window of the banded path (nodes)
 
 struct GroupStage {                        // per warp, shared memory
   double2 w0[RB][EMAX];
@@ -47,8 +48,13 @@ struct GroupStage {                        // per warp, shared memory
   double2 w2[RB][NS];
   int off0[EMAX], off1[EMAX];
   double c[RB];
-  int roff[2][RB][EMAX];                   // the rows' own lists, when they have to be merged
-  double2 rw[2][RB][EMAX];
+  union {
+    struct {                               // the rows' own lists, when they have to be merged
+      int roff[2][RB][EMAX];
+      double2 rw[2][RB][EMAX];
+    };
+    double2 W2[WMAX2][RB];                 // dense dimension-2 weights of a wide union window (after the merge)
+  };
   int ucnt[2];
 };
 
@@ -139,6 +145,73 @@ __device__ __forceinline__ void contract_group(const GroupStage& st, int4 cref,
     }
 }
 
+// The contraction of a group whose dimension-2 weights were spread densely over the union window
+// wlo .. wlo+wwidth-1 (GroupStage::W2): weights broadcast from shared memory, every u / dP value of
+// the window loaded once for the four rows.  Not inlined: its registers stay out of the budget of
+// the static-slot paths.
+__device__ __noinline__ void contract_wide(const GroupStage& st, int n0e, int n1e,
+                                           const double* __restrict__ u,
+                                           const double* __restrict__ d0,
+                                           const double* __restrict__ d1,
+                                           const double* __restrict__ d2, int wlo, int wwidth,
+                                           double* __restrict__ acc) {
+#pragma unroll
+      for (int r = 0; r < RB; ++r) acc[r] = st.c[r];
+      for (int e0 = 0; e0 < n0e; ++e0) {
+        double Ap[RB], B0p[RB];
+#pragma unroll
+        for (int r = 0; r < RB; ++r) Ap[r] = B0p[r] = 0.0;
+        for (int e1 = 0; e1 < n1e; ++e1) {
+          const int o = st.off0[e0] + st.off1[e1] + wlo * FK_CW;
+          const double* pu = u + o;
+          const double* p0 = d0 + o;
+          const double* p1 = d1 + o;
+          const double* p2 = d2 + o;
+          asm volatile("" : "+l"(pu), "+l"(p0), "+l"(p1), "+l"(p2));
+          double A[RB], B0[RB], B1[RB];
+#pragma unroll
+          for (int r = 0; r < RB; ++r) A[r] = B0[r] = B1[r] = 0.0;
+          // two window nodes per iteration; an odd window reads one node past its end with the zero
+          // weights W2 was cleared to (a node of the next line, chunk or a guard row)
+          for (int q = 0; q < wwidth; q += 2) {
+            double U[2], D0[2], D1[2], D2[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              U[h] = pu[h * FK_CW]; D0[h] = p0[h * FK_CW]; D1[h] = p1[h * FK_CW]; D2[h] = p2[h * FK_CW];
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int r = 0; r < RB; ++r) {
+                const double2 w = st.W2[q + h][r];
+                A[r] = fma(w.x, U[h], A[r]);
+                A[r] = fma(w.y, D2[h], A[r]);
+                B0[r] = fma(w.x, D0[h], B0[r]);
+                B1[r] = fma(w.x, D1[h], B1[r]);
+              }
+            pu += 2 * FK_CW; p0 += 2 * FK_CW; p1 += 2 * FK_CW; p2 += 2 * FK_CW;
+          }
+#pragma unroll
+          for (int r = 0; r < RB; ++r) {
+            const double2 w1 = st.w1[r][e1];
+            Ap[r] = fma(w1.x, A[r], Ap[r]);
+            Ap[r] = fma(w1.y, B1[r], Ap[r]);
+            B0p[r] = fma(w1.x, B0[r], B0p[r]);
+          }
+        }
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+          const double2 w0 = st.w0[r][e0];
+          acc[r] = fma(w0.x, Ap[r], acc[r]);
+          acc[r] = fma(w0.y, B0p[r], acc[r]);
+        }
+      }
+}
+
+// WIDE: with the banded dimension-2 path (instantiated for grids whose last dimension is non-uniform;
+// on uniform grids the few rows that reach beyond H2 nodes take the row-at-a-time path and the
+// kernel keeps the register budget of the static-slot paths)
+template <bool WIDE>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
               const double* __restrict__ dP, double* __restrict__ Pnew, int n_chunks, int chunk0,
@@ -180,7 +253,8 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     return;
   }
   // every load of the stage is issued before anything is compared (one round of latency)
-  bool ok = !g.periodic[2];                             // a wrapped run has no static slots
+  bool ok = true;                                       // dimension-0 / 1 lists fit the blocked paths
+  bool ok2 = !g.periodic[2];                            // dimension 2 fits the static slots (a wrapped run has none)
   bool same = true;                                     // rows put their dimension-0 / 1 entries on the same nodes
   {
     const int dim = lane >> 4, e = lane & (EMAX - 1);   // lanes 0..15: dimension 0, 16..31: 1
@@ -197,7 +271,8 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
       off01[r] = INT_MAX;                               // "no entry": sorts last in the merge
       off2[r] = 0;
       w01[r] = w2[r] = make_double2(0.0, 0.0);
-      ok = ok && cnt[r].x <= EMAX && cnt[r].y <= EMAX && cnt[r].z <= NS;
+      ok = ok && cnt[r].x <= EMAX && cnt[r].y <= EMAX;
+      ok2 = ok2 && cnt[r].z <= NS;
       if (!dir && ne <= EMAX && e < ne) { off01[r] = op.off[row + q]; w01[r] = op.w[row + q]; }
       if (!dir && lane < cnt[r].z && lane < NS) { off2[r] = op.off[row + q2]; w2[r] = op.w[row + q2]; }
       if (lane == r && r < rows) cr = op.c[jb + r];
@@ -212,6 +287,7 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
       if (!(cnt[r].w & FK_ROW_DIRICHLET)) same = same && off01[r] == oref;
     same = __all_sync(0xffffffffu, same);
     ok = __all_sync(0xffffffffu, ok);
+    ok2 = __all_sync(0xffffffffu, ok2);
     __syncwarp();
     if (same) {
       if (dim) st.off1[e] = oref; else st.off0[e] = oref;
@@ -254,16 +330,47 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
 #pragma unroll
     for (int r = 0; r < RB; ++r) {
       if (cnt[r].w & FK_ROW_DIRICHLET) continue;
-      if (ok && lane < cnt[r].z && lane < NS) {
+      if (ok && ok2 && lane < cnt[r].z && lane < NS) {
         // dimension 2: entries -> slots around the row's own node (its stride is 1 node)
         const int t = off2[r] / FK_CW - (i2b + r) + H2;
         if (t >= 0 && t < NS) st.w2[r][t] = w2[r];
-        else ok = false;
+        else ok2 = false;
       }
     }
   }
   ok = __all_sync(0xffffffffu, ok);
+  ok2 = __all_sync(0xffffffffu, ok2);
   __syncwarp();
+
+  // ---- rows that reach beyond H2 nodes along dimension 2 (a fine non-uniform grid: the paper's radial
+  // grid): if their union window is a band of at most WMAX2 nodes, spread the
+  // dimension-2 weights densely over it in shared memory (zero where a row has no entry) and contract
+  // the four rows together on the window -- every u / dP value still loaded once per group
+  int wlo = INT_MAX, whi = -1;
+  bool wide = WIDE && ok && !ok2 && !g.periodic[2];
+  if (wide) {
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      if ((cnt[r].w & FK_ROW_DIRICHLET) || cnt[r].z == 0) continue;
+      const int* __restrict__ o = op.off + (size_t)(jb + r) * g.RS + g.qoff[2];
+      wlo = min(wlo, o[0] / FK_CW);
+      whi = max(whi, o[cnt[r].z - 1] / FK_CW);
+    }
+    wide = whi >= wlo && whi - wlo + 1 <= WMAX2;
+  }
+  const int wwidth = whi - wlo + 1;
+  if (wide) {
+    for (int k = lane; k < WMAX2 * RB; k += 32) (&st.W2[0][0])[k] = make_double2(0.0, 0.0);
+    __syncwarp();
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      if (cnt[r].w & FK_ROW_DIRICHLET) continue;
+      const size_t row = (size_t)(jb + r) * g.RS + g.qoff[2];
+      for (int e = lane; e < cnt[r].z; e += 32) st.W2[op.off[row + e] / FK_CW - wlo][r] = op.w[row + e];
+    }
+    __syncwarp();
+  }
+  ok = ok && ok2;                                        // the static-slot blocked path
 
   // ---- which dimension-2 slots carry a weight in any row decides the variant of the blocked path
   unsigned tmask = 0;
@@ -301,6 +408,15 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     const double* __restrict__ d1 = d0 + field;
     const double* __restrict__ d2 = d1 + field;
     double* __restrict__ out = Pnew + (size_t)chunk * chunk_elems + (size_t)jb * FK_CW + lane;
+    if (wide) {
+      // ---- banded along dimension 2: dense window, weights broadcast from shared memory
+      double acc[RB];
+      contract_wide(st, cref.x, cref.y, u, d0, d1, d2, wlo, wwidth, acc);
+#pragma unroll
+      for (int r = 0; r < RB; ++r)
+        if (r < rows && active) out[r * FK_CW] = (cnt[r].w & FK_ROW_DIRICHLET) ? st.c[r] : acc[r];
+      continue;
+    }
     if (!ok) {
       // ---- row-at-a-time path
 #pragma unroll
@@ -339,6 +455,7 @@ cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* P
   const int G2 = (g.n[2] + RB - 1) / RB;
   const int NT1 = (g.n[1] + WARPS - 1) / WARPS;
   dim3 block(FK_CW, WARPS), grid((unsigned)((long long)g.n[0] * NT1 * G2), (unsigned)((chunk1 - chunk0 + CPB - 1) / CPB));
-  fk_rowblock3d<<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, chunk1, n, N, G2, NT1);
+  if (g.uniform[2]) fk_rowblock3d<false><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, chunk1, n, N, G2, NT1);
+  else fk_rowblock3d<true><<<grid, block, 0, s>>>(g, op, Pold, dP, Pnew, n_chunks, chunk0, chunk1, n, N, G2, NT1);
   return cudaGetLastError();
 }
