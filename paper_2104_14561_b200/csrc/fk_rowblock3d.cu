@@ -288,6 +288,7 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     same = __all_sync(0xffffffffu, same);
     ok = __all_sync(0xffffffffu, ok);
     ok2 = __all_sync(0xffffffffu, ok2);
+    if (!WIDE) ok = ok && ok2;          // no banded path: such a group goes row by row, skip the merge
     __syncwarp();
     if (same) {
       if (dim) st.off1[e] = oref; else st.off0[e] = oref;
