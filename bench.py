@@ -78,8 +78,8 @@ TRAFFIC = {
         "launch": "step n = 424 of config 3's grid (601 active columns, 20 chunks)",
         "profile": "profiles/r2_fused2d_ncu_full.md"},
     ("cfg5_runaway_3d", "rowblock"): {
-        "source": "fk_rowblock3d.cu", "source_sha1": "381b71ef76608be20cd5cd6ab96d61c04f5fe381",
-        "dram_bytes": 5371195000, "algorithmic_bytes": 646216704,
+        "source": "fk_rowblock3d.cu", "source_sha1": "a998d9565f0f1da17ad5dcf8fdd808dc1cbd7856",
+        "dram_bytes": 5374427000, "algorithmic_bytes": 646216704,
         "launch": "step n = 48 of config 5's grid (49 active columns in 3 chunks: half of the lanes idle; this "
                   "path also reads three slope fields: 40 B per update, and the factored rows per chunk group)",
         "profile": "profiles/r2_cfg5_kernels_ncu_full.md"},
