@@ -99,6 +99,47 @@ def test_2d_far_rows_only_and_mixed(fk, oracle_mod):
     check(fk, oracle_mod, wl)
 
 
+def test_2d_lines_handed_over_at_either_end(fk, oracle_mod):
+    """The per-step plan (fk_api.cu plan_2d) gives the lines at either end of dimension 0 on which
+    at least half of the rows are far to fk_far2d whole and runs the fused kernel on the rest: reach
+    that grows towards the LAST lines (suffix hand-over), towards both ends, and a CLAMP face in
+    dimension 0 (the first line is updated, not Dirichlet).  All kernels must run, result vs oracle."""
+    B, solve = fk
+    lin = lambda n: np.linspace(-1.0, 1.0, n)
+    for name, kinds, shape in (("top", [[A, A], [A, C]], lambda t: t ** 3),
+                               ("both", [[C, A], [C, C]], lambda t: (2 * t - 1) ** 4)):
+        wl = make("plan_" + name, [lin(57), lin(45)], 4e-3, 35, [6, 8], kinds, [[1, 0], [0, 1]], 41,
+                  drift=1.0, sigma=0.05)
+        j0 = np.repeat(np.arange(57), 45)
+        scale = 1.0 + 14.0 * shape(j0 / 56.0)
+        base = wl.coeffs
+
+        def coeffs(n, base=base, scale=scale):
+            b, s = base(n)
+            s = s.copy()
+            s[1] *= scale
+            return b, s
+        wl.coeffs = coeffs
+        ref = oracle_mod.Oracle(wl).algorithm1()
+        ctx = solve.create_for(wl, wl.N)
+        try:
+            B.fk_profile(ctx, True)
+            solve.evolve_loaded(ctx, wl, wl.N)
+            got = np.empty((wl.N + 1, wl.J))
+            B.fk_read(ctx, 0, wl.N + 1, got)
+            prof = B.fk_profile_read(ctx)
+            upd = B.fk_profile_updates(ctx)
+        finally:
+            B.fk_destroy(ctx)
+        assert prof["fused"][1] == wl.N and prof["far2d"][1] == wl.N, prof
+        # every updated row is owned by exactly one of the two kernels
+        n_upd = (57 - (kinds[0][0] == A) - (kinds[0][1] == A)) * (45 - (kinds[1][0] == A) - (kinds[1][1] == A))
+        assert upd["fused"] + upd["far2d"] == pytest.approx(n_upd * wl.N * (wl.N + 1) / 2)
+        assert upd["far2d"] > 0.05 * upd["fused"]
+        err = float(np.abs(got - ref).max())
+        assert err <= TOL, f"{wl.name}: max abs error {err:.3e}"
+
+
 @pytest.mark.parametrize("idx,nprefix", [(2, 24), (3, 12)])
 def test_full_size_config_prefix_and_invariants(fk, oracle_mod, idx, nprefix):
     import torch
