@@ -155,6 +155,42 @@ int fk_read(fk_ctx* c, int m0, int m1, double* out, int mem);
  * fk_read; synchronises the stream when `mem` is FK_MEM_HOST. */
 int fk_reduce(fk_ctx* c, const double* weights, int m0, int m1, double* out, int mem);
 
+/* fk_reduce without any device allocation: same sums, same fixed summation order (the results are
+ * bit-identical to fk_reduce on device buffers), for callers that must not -- or cannot -- call
+ * cudaMalloc at this point.  Who that is: a program whose device memory is already fully handed out
+ * (a framework's caching allocator that has taken the rest of the GPU, or simply config-5-sized
+ * contexts that leave no room: a late cudaMalloc there fails with out-of-memory), and a program
+ * that reduces inside a loop it cannot afford to stall (cudaMalloc and cudaFree make the whole
+ * device wait, other streams included; fk_reduce grows its scratch with them whenever a call needs
+ * more than the one before).
+ *
+ * How: fk_reduce's only scratch, the per-block partial sums of its first pass, sits in a fixed
+ * array compiled into the library: FK_REDUCE_STATIC_MAX_CHUNKS_ABI x 64 x 32 doubles = 1 MiB of
+ * device memory on every GPU that loads the library, kept until the process exits whether or not
+ * this call is ever used.  That bounds what one call can take: the columns m0..m1-1 may touch at
+ * most FK_REDUCE_STATIC_MAX_CHUNKS_ABI = 64 of the 32-column chunks (chunk = m / 32), i.e. any range
+ * of up to 2017 columns, 2048 when m0 is a multiple of 32 (configs 1, 2, 3 and 5 in one call;
+ * config 4's 5001 columns in three).  A wider range is refused with FK_EINVAL and a message that
+ * says so; nothing is launched then.
+ *
+ * weights[J] and out[m1-m0] are the caller's and must both be DEVICE memory on the context's device
+ * (anything else is refused with FK_EINVAL: there is no room to stage a host array without
+ * allocating).  The call queues two kernels on the context's stream and returns without waiting;
+ * `out` is ready when the stream has passed them.  State rules and shard behaviour as fk_reduce.
+ *
+ * Shared state, read this: the array belongs to the library, not to a context.  Every call on a
+ * device, from whatever context or stream, uses the same memory, so two calls whose kernels can be
+ * on the GPU at the same time (different streams, different contexts, different threads) corrupt
+ * each other's sums -- keep them on one stream or order them with events.  Calls that run one
+ * after the other are safe: nothing in the array needs to start at zero, the second pass reads only
+ * what the first pass of the same call wrote, so leftovers of an earlier call never count.
+ *
+ * First call on each device: looks up the device address of the array (cudaGetSymbolAddress, once
+ * per device, with that device current) and remembers it; later calls only launch.  Make that
+ * first call during start-up, before any stream capture begins on that device. */
+#define FK_REDUCE_STATIC_MAX_CHUNKS_ABI 64
+int fk_reduce_static(fk_ctx* c, const double* weights, int m0, int m1, double* out);
+
 /* Synchronise the context's stream and report what the device found since the last fk_reset:
  * FK_OK, or FK_EINVAL with fk_last_error naming the first kind of bad coefficient (negative
  * sigma at an updated node; NaN / Inf with FK_FLAG_VALIDATE). */

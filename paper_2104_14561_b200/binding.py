@@ -1,7 +1,7 @@
 """ctypes binding of the C ABI in include/fk.h (libfk_b200.so): argument marshalling only.
 
 Same names as the C entry points (`fk_create`, `fk_set_coeffs`, `fk_set_coeffs_range`,
-`fk_evolve`, `fk_reset`, `fk_read`, `fk_reduce`, `fk_check`, `fk_profile`, `fk_profile_read`,
+`fk_evolve`, `fk_reset`, `fk_read`, `fk_reduce`, `fk_reduce_static`, `fk_check`, `fk_profile`, `fk_profile_read`,
 `fk_profile_updates`, `fk_work`, `fk_peak_fp64`, `fk_launch_count`, `fk_destroy`,
 `fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
 pointers) or torch CUDA tensors (device pointers); every step of the path runs in the CUDA
@@ -19,6 +19,7 @@ FK_FACE_ABSORB, FK_FACE_CLAMP, FK_FACE_PERIODIC = 0, 1, 2
 FK_MEM_HOST, FK_MEM_DEVICE = 0, 1
 FK_ALL_STEPS = -1
 FK_MAX_Q = 32
+FK_REDUCE_STATIC_MAX_CHUNKS = 64
 FK_FLAG_VALIDATE = 1
 FK_FLAG_WEIGHTED_SLOPES = 2
 FK_FLAG_MULTISTEP = 4
@@ -28,7 +29,7 @@ KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock", "far2d", "
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.so")
 
 EXPORTS = ("fk_create", "fk_set_coeffs", "fk_set_coeffs_range", "fk_evolve", "fk_reset",
-           "fk_read", "fk_reduce", "fk_check", "fk_profile", "fk_profile_read",
+           "fk_read", "fk_reduce", "fk_reduce_static", "fk_check", "fk_profile", "fk_profile_read",
            "fk_profile_updates", "fk_work", "fk_peak_fp64", "fk_launch_count", "fk_destroy",
            "fk_last_error", "fk_gauss_hermite")
 
@@ -67,6 +68,7 @@ def lib():
         L.fk_reset.argtypes = [vp]
         L.fk_read.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.fk_reduce.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int]
+        L.fk_reduce_static.argtypes = [vp, vp, C.c_int, C.c_int, vp]
         L.fk_check.argtypes = [vp]
         L.fk_profile.argtypes = [vp, C.c_int]
         L.fk_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
@@ -188,6 +190,19 @@ def fk_reduce(ctx, weights, m0, m1, out):
     if mw != mo:
         raise ValueError("weights and out must both be host or both be device arrays")
     _check(ctx, lib().fk_reduce(ctx, pw, int(m0), int(m1), po, mo))
+    return out
+
+
+def fk_reduce_static(ctx, weights, m0, m1, out):
+    """fk_reduce for callers that cannot allocate device memory: weights [J] and out [m1-m0] must be
+    CUDA tensors, the range may touch at most FK_REDUCE_STATIC_MAX_CHUNKS 32-column chunks, and the
+    partial sums go to a fixed array inside the library that all calls on a device share (do not let
+    two calls overlap on the GPU).  Asynchronous on the context's stream; see include/fk.h."""
+    pw, mw, kw = _buffer(weights)
+    po, mo, ko = _buffer(out, m1 - m0)
+    if ko is not out:
+        raise TypeError("out must be a contiguous float64 CUDA tensor")
+    _check(ctx, lib().fk_reduce_static(ctx, pw, int(m0), int(m1), po))
     return out
 
 

@@ -863,6 +863,38 @@ int fk_reduce(fk_ctx* c, const double* weights, int m0, int m1, double* out, int
   return FK_OK;
 }
 
+// fk_reduce for callers that cannot allocate device memory (include/fk.h): device buffers only, the
+// partial sums live in the library's fixed scratch array.  No cudaMalloc / cudaFree here or below.
+int fk_reduce_static(fk_ctx* c, const double* weights, int m0, int m1, double* out) {
+  if (!c) return FK_EINVAL;
+  if (!weights || !out) return fail(c, FK_EINVAL, "weights or out is NULL");
+  if (m0 < 0 || m1 > c->N + 1 || m0 >= m1) return fail(c, FK_EINVAL, "need 0 <= m0 < m1 <= N+1");
+  const int chunks = (m1 - 1) / FK_CW - m0 / FK_CW + 1;
+  if (chunks > FK_REDUCE_STATIC_MAX_CHUNKS) {
+    char msg[200];
+    std::snprintf(msg, sizeof msg,
+                  "fk_reduce_static: columns %d..%d touch %d chunks of 32 columns, the fixed scratch "
+                  "holds %d; split the range or use fk_reduce",
+                  m0, m1 - 1, chunks, FK_REDUCE_STATIC_MAX_CHUNKS);
+    return fail(c, FK_EINVAL, msg);
+  }
+  static_assert(FK_REDUCE_STATIC_MAX_CHUNKS == FK_REDUCE_STATIC_MAX_CHUNKS_ABI, "fk.h and fk_internal.h disagree");
+  if (c->n_next != 0 && m1 > 1) return fail(c, FK_ESTATE, "columns other than 0 are final only after fk_evolve reached n_to = 0");
+  if (*c->h_status) return fail(c, FK_EINVAL, status_text(*c->h_status));
+  DeviceGuard guard(c->device);
+  // both buffers are read / written by kernels: a host pointer would fault there, refuse it here
+  const void* ptrs[2] = {weights, out};
+  for (const void* p : ptrs) {
+    cudaPointerAttributes at;
+    FK_CUDA(c, cudaPointerGetAttributes(&at, p));
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+      return fail(c, FK_EINVAL, "fk_reduce_static: weights and out must be device memory");
+  }
+  FK_CUDA(c, fk_launch_reduce_static(c->g, c->d_P[c->cur], weights, m0, m1, out, c->device, c->stream));
+  c->launches += 2;
+  return FK_OK;
+}
+
 int fk_profile_updates(fk_ctx* c, double* updates) {
   if (!c) return FK_EINVAL;
   if (!updates) return fail(c, FK_EINVAL, "updates is NULL");

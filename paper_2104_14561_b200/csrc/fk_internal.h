@@ -144,6 +144,12 @@ cudaError_t fk_launch_rowblock3d(const FkGrid& g, FkOperator op, const double* P
 #define FK_RED_BLOCKS 64
 cudaError_t fk_launch_reduce(const FkGrid& g, const double* P, const double* w, int m0, int m1,
                              double* partial, double* out, cudaStream_t s);
+// the same reduction with the partial sums in a fixed array inside the library image (no allocation):
+// at most FK_REDUCE_STATIC_MAX_CHUNKS chunks touched by [m0, m1); `device` must be the current
+// device; the first call on a device looks up the array's address on it (fk_kernels.cu)
+#define FK_REDUCE_STATIC_MAX_CHUNKS 64   // == FK_REDUCE_STATIC_MAX_CHUNKS_ABI of include/fk.h
+cudaError_t fk_launch_reduce_static(const FkGrid& g, const double* P, const double* w, int m0,
+                                    int m1, double* out, int device, cudaStream_t s);
 cudaError_t fk_launch_gather_columns(const FkGrid& g, const double* P, int m0, int m1,
                                      double* out, cudaStream_t s);
 

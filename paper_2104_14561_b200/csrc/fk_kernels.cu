@@ -14,6 +14,8 @@
 // whole box, ...), and the operator row is warp-uniform, so it is fetched by broadcast loads.
 #include "fk_device.cuh"
 
+#include <mutex>
+
 namespace {
 
 using fkd::unravel;
@@ -600,6 +602,57 @@ cudaError_t fk_launch_reduce(const FkGrid& g, const double* P, const double* w, 
   dim3 block(32, 8), grid(FK_RED_BLOCKS, (unsigned)(c1 - c0));
   fk_reduce_partial<<<grid, block, 0, s>>>(g, P, w, c0, partial);
   cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  fk_reduce_final<<<(unsigned)(c1 - c0), 32, 0, s>>>(g, partial, c0, m0, m1, out);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// fk_reduce_static (include/fk.h): the same two passes as fk_launch_reduce, with the partial sums of
+// pass 1 kept in a fixed array that is part of the library image instead of in a buffer from
+// cudaMalloc.  FK_REDUCE_STATIC_MAX_CHUNKS x FK_RED_BLOCKS x 32 doubles = 1 MiB, held by every GPU
+// that loads the library until the process exits.
+//
+// In HOST code the name `fk_reduce_static_scratch` is only a handle for the runtime, not a device
+// address, so it must never be handed to a kernel as it is: the address the kernels get comes from
+// cudaGetSymbolAddress, asked once per device with that device current (every device has its own
+// copy of the array at its own address) and remembered here.
+//
+// Nothing in the array has to start at zero: pass 2 reads exactly the slots pass 1 of the same
+// call wrote (a shard skips both passes for the chunks it does not own), so whatever an earlier
+// call left behind is never looked at.
+// ------------------------------------------------------------------------------------------
+static __device__ __align__(256) double
+    fk_reduce_static_scratch[(size_t)FK_REDUCE_STATIC_MAX_CHUNKS * FK_RED_BLOCKS * FK_CW];
+
+#define FK_STATIC_MAX_DEVICES 64
+static std::mutex g_static_mutex;
+static double* g_static_scratch_ptr[FK_STATIC_MAX_DEVICES];   // per device ordinal, NULL = not asked yet
+
+cudaError_t fk_launch_reduce_static(const FkGrid& g, const double* P, const double* w, int m0,
+                                    int m1, double* out, int device, cudaStream_t s) {
+  const int c0 = m0 / FK_CW, c1 = (m1 - 1) / FK_CW + 1;
+  if (c1 - c0 > FK_REDUCE_STATIC_MAX_CHUNKS || device < 0 || device >= FK_STATIC_MAX_DEVICES)
+    return cudaErrorInvalidValue;
+  int cur = -1;
+  cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return e;
+  if (cur != device) return cudaErrorInvalidDevice;          // the caller makes `device` current
+  double* partial = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_scratch_ptr[device]) {                     // set-up: first call on this device
+      void* ptr = nullptr;
+      e = cudaGetSymbolAddress(&ptr, fk_reduce_static_scratch);
+      if (e != cudaSuccess) return e;
+      if (!ptr) return cudaErrorInvalidSymbol;
+      g_static_scratch_ptr[device] = static_cast<double*>(ptr);
+    }
+    partial = g_static_scratch_ptr[device];
+  }
+  dim3 block(32, 8), grid(FK_RED_BLOCKS, (unsigned)(c1 - c0));
+  fk_reduce_partial<<<grid, block, 0, s>>>(g, P, w, c0, partial);
+  e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   fk_reduce_final<<<(unsigned)(c1 - c0), 32, 0, s>>>(g, partial, c0, m0, m1, out);
   return cudaGetLastError();
