@@ -60,12 +60,12 @@ SM_CLOCK_HZ = 1.965e9          # clocks.max.sm of the B200 (the run's own clock 
 # the one profiled (sha1 below); otherwise `traffic` is null rather than stale.
 TRAFFIC = {
     ("cfg4_runaway_2d", "far2d"): {
-        "source": "fk_far2d.cu", "source_sha1": "bb01a21dbabd7b31c53ace01530a2919c010bbed",
-        "dram_bytes": 450597632, "algorithmic_bytes": 193100000,
+        "source": "fk_far2d.cu", "source_sha1": "45e1659936146f32bc7e8d238ca631e4ee91c23f",
+        "dram_bytes": 455071488, "algorithmic_bytes": 193100000,
         "launch": "step n = 424 of config 4's grid (601 active columns, 20 chunks, about 20.1e3 rows: 17.8e3 far rows "
                   "and the near rows of the lines handed over whole); this path also "
                   "reads the two slope fields: 32 B per update",
-        "profile": "profiles/r2_cfg4_kernels_ncu_full.md"},
+        "profile": "profiles/r3_cfg4_cfg5_kernels_ncu_full.md"},
     ("cfg4_runaway_2d", "fused"): {
         "source": "fk_fused2d.cu", "source_sha1": "a69b7c46b8f12346ea4808a2f39802e3470c1529",
         "dram_bytes": 650159104, "algorithmic_bytes": 578100000,
@@ -78,11 +78,12 @@ TRAFFIC = {
         "launch": "step n = 424 of config 3's grid (601 active columns, 20 chunks)",
         "profile": "profiles/r2_fused2d_ncu_full.md"},
     ("cfg5_runaway_3d", "rowblock"): {
-        "source": "fk_rowblock3d.cu", "source_sha1": "a998d9565f0f1da17ad5dcf8fdd808dc1cbd7856",
-        "dram_bytes": 5374427000, "algorithmic_bytes": 646216704,
-        "launch": "step n = 48 of config 5's grid (49 active columns in 3 chunks: half of the lanes idle; this "
-                  "path also reads three slope fields: 40 B per update, and the factored rows per chunk group)",
-        "profile": "profiles/r2_cfg5_kernels_ncu_full.md"},
+        "source": "fk_rowblock3d.cu", "source_sha1": "e37193f408aa37f583ca81e12153df066f980be5",
+        "dram_bytes": 12413479000, "algorithmic_bytes": 2954133504,
+        "launch": "step n = 32 of config 5's grid evolved for 255 steps (224 active columns = 7 FULL chunks, every lane "
+                  "busy: 16 B x 824256 updated nodes x 224 columns); this path also reads three slope fields "
+                  "(40 B per update) and the factored rows once per group of two chunks",
+        "profile": "profiles/r3_cfg4_cfg5_kernels_ncu_full.md"},
 }
 
 
@@ -403,6 +404,19 @@ def profile_pass(B, torch, runner, streamed):
     return prof, step_ms, upd, work
 
 
+def compact(x, digits=5):
+    """Floats rounded to `digits` significant digits, recursively: keeps the per_config block (one
+    entry per configuration) short enough that a record which keeps only the tail of the line still
+    holds every configuration."""
+    if isinstance(x, float):
+        return float(f"{x:.{digits}g}")
+    if isinstance(x, dict):
+        return {k: compact(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [compact(v, digits) for v in x]
+    return x
+
+
 def run_cuda(args, wl, rank, world):
     import torch
     import torch.distributed as dist
@@ -526,8 +540,8 @@ def run_cuda(args, wl, rank, world):
                 per_config[w2.name] = {
                     "grid": list(w2.n), "N": w2.N, "prefix_of_N": W.config(7).N if idx == 7 else None, "updates": w2.updates, "ms_per_evolution": ms2,
                     "updates_per_s": w2.updates / (ms2 * 1e-3),
-                    "coefficients": "resident in HBM" if res2 else f"streamed through a ring of {RING_SLOTS} slots "
-                                    "(generated on the host and uploaded between the timed fk_evolve pieces)",
+                    # "ring": generated on the host and uploaded between the timed fk_evolve pieces
+                    "coefficients": "resident" if res2 else f"ring{RING_SLOTS}",
                     "dominant": {k: rl2[k] for k in ("kernel", "bound", "frac", "share_of_step")},
                     "hbm_frac": rl2["hbm"]["frac"], "fp64_frac": rl2["fp64"]["frac"],
                     "whole_step": rl2["whole_step"], "class_ms": rl2["class_ms"]}
@@ -555,7 +569,7 @@ def run_cuda(args, wl, rank, world):
         "roofline": rl,
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "per_config": per_config,
+        "per_config": compact(per_config),
     }
     if e2e is not None:
         line["e2e"] = e2e

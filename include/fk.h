@@ -50,7 +50,13 @@ enum { FK_OK = 0, FK_EINVAL = 1, FK_ENOMEM = 2, FK_ECUDA = 3, FK_ESTATE = 4 };
  *         same coefficients).  Problems with a periodic dimension run on the generic kernels. */
 enum { FK_FACE_ABSORB = 0, FK_FACE_CLAMP = 1, FK_FACE_PERIODIC = 2 };
 
-enum { FK_MEM_HOST = 0, FK_MEM_DEVICE = 1 };
+/* FK_MEM_HOST_PINNED (fk_set_coeffs / fk_set_coeffs_range only): a page-locked HOST buffer that the
+ * caller keeps valid and unmodified until the context's stream has reached the copy, exactly like a
+ * device buffer.  The call then only queues the copies and returns without synchronising, so the
+ * upload of the next ring piece overlaps the kernels of the current one (config 5 streams 81 GB of
+ * coefficients through its ring).  With pageable memory the copies are still correct but no longer
+ * asynchronous. */
+enum { FK_MEM_HOST = 0, FK_MEM_DEVICE = 1, FK_MEM_HOST_PINNED = 2 };
 
 /* fk_params.flags */
 enum {
@@ -64,6 +70,9 @@ enum {
                             operators per pass over P: SURVEY.md section 8(f)'s temporal blocking).
                             Same results up to summation order.  Off by default: measured faster
                             only on short lines */
+  FK_FLAG_COUNT_PATHS = 8, /* testing aid: count, per group of four rows and step, which contraction path
+                            of the blocked 2-D / 3-D apply kernels the group took (fk_paths); one
+                            predicated atomic per group */
   FK_FLAG_WEIGHTED_SLOPES = 2  /* nodal slopes by the Fritsch-Carlson weighted harmonic mean
                             (ref [17]; R22) instead of Eq. 15 as printed:
                             (w1+w2)/(w1/d_{j-1} + w2/d_j), w1 = 2h_j + h_{j-1}, w2 = h_j + 2h_{j-1};
@@ -116,7 +125,8 @@ int fk_create(const fk_params* p, fk_ctx** out);
  * columns computed from such a step are undefined.  Non-finite values are reported the same
  * way when FK_FLAG_VALIDATE is set, and are undefined (they propagate as NaN) otherwise.
  * Copies are stream-ordered; a host buffer may be reused when the call returns (the call
- * synchronises the stream for host sources). */
+ * synchronises the stream for FK_MEM_HOST sources; FK_MEM_HOST_PINNED sources are not waited for,
+ * see above). */
 int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int mem);
 
 /* Same for `count` consecutive steps step0..step0+count-1: b and sigma are [count][d][J].
@@ -136,7 +146,9 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
  * step.  FK_EINVAL: a coefficient error found on the device by an earlier step (see fk_check). */
 int fk_evolve(fk_ctx* c, int n_from, int n_to);
 
-/* Refill P with chi and rewind to n = N; coefficient slots are kept. */
+/* Refill P with chi and rewind to n = N; coefficient slots are kept.  Clears the device's error
+ * flag (see fk_check); to do that safely the call waits until the kernels of the last fk_evolve on
+ * this context have finished (not for anything queued after them). */
 int fk_reset(fk_ctx* c);
 
 /* Copy columns m0..m1-1 out as out[(m1-m0)][J] (row m-m0 = P(t_m, .), node index fastest),
@@ -214,6 +226,19 @@ int fk_profile_read(fk_ctx* c, double* ms, long long* launches);
  * columns, Dirichlet rows excluded), host-side bookkeeping of fk_evolve: updates[FK_K_COUNT].
  * FK_K_ASSEMBLE counts operator rows assembled (one per updated node and step). */
 int fk_profile_updates(fk_ctx* c, double* updates);
+
+/* With FK_FLAG_COUNT_PATHS: how many (group of four adjacent rows, step) pairs each contraction path
+ * of the blocked apply kernels served since fk_create (synchronises the stream).  3-D (fk_rowblock3d):
+ * SAME = the four rows put their dimension-0 / 1 entries on the same nodes, static dimension-2 slots;
+ * MERGED = contracted on the union of the rows' entry lists; WIDE / WIDE_MERGED = the same two with
+ * the dimension-2 weights spread over a dense union window (rows that reach beyond two nodes along a
+ * non-uniform last dimension); ROWWISE = one row at a time (lists too long for the staging, a
+ * periodic or too wide dimension 2).  2-D (fk_far2d): BANDED = dense union window along dimension 1,
+ * SCATTERED = entry by entry.  FK_ESTATE without the flag.  The tests use it to prove that the path a
+ * parity case is meant for actually ran. */
+enum { FK_PATH_3D_SAME = 0, FK_PATH_3D_MERGED = 1, FK_PATH_3D_WIDE = 2, FK_PATH_3D_WIDE_MERGED = 3,
+       FK_PATH_3D_ROWWISE = 4, FK_PATH_2D_BANDED = 5, FK_PATH_2D_SCATTERED = 6, FK_PATH_COUNT = 8 };
+int fk_paths(fk_ctx* c, long long counts[FK_PATH_COUNT]);
 
 /* Algorithmic work of the steps evolved since the last fk_reset, counted on the device while the
  * operators are assembled (synchronises the stream): work[0] = node-step updates on rows the fused

@@ -2,7 +2,7 @@
 
 Same names as the C entry points (`fk_create`, `fk_set_coeffs`, `fk_set_coeffs_range`,
 `fk_evolve`, `fk_reset`, `fk_read`, `fk_reduce`, `fk_reduce_static`, `fk_check`, `fk_profile`, `fk_profile_read`,
-`fk_profile_updates`, `fk_work`, `fk_peak_fp64`, `fk_launch_count`, `fk_destroy`,
+`fk_profile_updates`, `fk_work`, `fk_paths`, `fk_peak_fp64`, `fk_launch_count`, `fk_destroy`,
 `fk_last_error`, `fk_gauss_hermite`).  Arrays may be numpy arrays (host
 pointers) or torch CUDA tensors (device pointers); every step of the path runs in the CUDA
 kernels behind the ABI.  There is no CPU fallback: a missing library raises.
@@ -16,13 +16,16 @@ import numpy as np
 
 FK_OK, FK_EINVAL, FK_ENOMEM, FK_ECUDA, FK_ESTATE = 0, 1, 2, 3, 4
 FK_FACE_ABSORB, FK_FACE_CLAMP, FK_FACE_PERIODIC = 0, 1, 2
-FK_MEM_HOST, FK_MEM_DEVICE = 0, 1
+FK_MEM_HOST, FK_MEM_DEVICE, FK_MEM_HOST_PINNED = 0, 1, 2
 FK_ALL_STEPS = -1
 FK_MAX_Q = 32
 FK_REDUCE_STATIC_MAX_CHUNKS = 64
 FK_FLAG_VALIDATE = 1
 FK_FLAG_WEIGHTED_SLOPES = 2
 FK_FLAG_MULTISTEP = 4
+FK_FLAG_COUNT_PATHS = 8
+PATHS = ("3d_same", "3d_merged", "3d_wide", "3d_wide_merged", "3d_rowwise", "2d_banded", "2d_scattered")
+FK_PATH_COUNT = 8
 FK_K_ASSEMBLE, FK_K_SLOPES, FK_K_APPLY, FK_K_FUSED, FK_K_ROWBLOCK, FK_K_FAR2D, FK_K_LINE1D, FK_K_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
 KERNEL_CLASSES = ("assemble", "slopes", "apply", "fused", "rowblock", "far2d", "line1d")
 
@@ -30,7 +33,7 @@ LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfk_b200.
 
 EXPORTS = ("fk_create", "fk_set_coeffs", "fk_set_coeffs_range", "fk_evolve", "fk_reset",
            "fk_read", "fk_reduce", "fk_reduce_static", "fk_check", "fk_profile", "fk_profile_read",
-           "fk_profile_updates", "fk_work", "fk_peak_fp64", "fk_launch_count", "fk_destroy",
+           "fk_profile_updates", "fk_work", "fk_paths", "fk_peak_fp64", "fk_launch_count", "fk_destroy",
            "fk_last_error", "fk_gauss_hermite")
 
 
@@ -74,6 +77,7 @@ def lib():
         L.fk_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.fk_profile_updates.argtypes = [vp, dp]
         L.fk_work.argtypes = [vp, dp]
+        L.fk_paths.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.fk_peak_fp64.argtypes = [C.c_int, vp, C.c_int, dp, dp]
         L.fk_launch_count.argtypes = [vp]
         L.fk_launch_count.restype = C.c_longlong
@@ -155,11 +159,17 @@ def fk_set_coeffs(ctx, step, b, sigma):
     _check(ctx, lib().fk_set_coeffs(ctx, int(step), pb, ps, mb))
 
 
-def fk_set_coeffs_range(ctx, step0, count, b, sigma):
+def fk_set_coeffs_range(ctx, step0, count, b, sigma, pinned_async=False):
+    """pinned_async: b and sigma are page-locked torch CPU tensors that the caller keeps alive and
+    unchanged until the context's stream has passed the copies (FK_MEM_HOST_PINNED: no sync)."""
     pb, mb, kb = _buffer(b)
     ps, ms, ks = _buffer(sigma)
     if mb != ms:
         raise ValueError("b and sigma must both be host or both be device arrays")
+    if pinned_async:
+        if mb != FK_MEM_HOST or not (hasattr(b, "is_pinned") and b.is_pinned() and sigma.is_pinned()):
+            raise ValueError("pinned_async needs page-locked torch CPU tensors")
+        mb = FK_MEM_HOST_PINNED
     _check(ctx, lib().fk_set_coeffs_range(ctx, int(step0), int(count), pb, ps, mb))
 
 
@@ -235,6 +245,13 @@ def fk_work(ctx):
     w = (C.c_double * 4)()
     _check(ctx, lib().fk_work(ctx, w))
     return {"updates_near": w[0], "fma_near": w[1], "updates_other": w[2], "fma_other": w[3]}
+
+
+def fk_paths(ctx):
+    """-> {path: (group of four rows, step) pairs it served}; needs FK_FLAG_COUNT_PATHS at fk_create."""
+    n = (C.c_longlong * FK_PATH_COUNT)()
+    _check(ctx, lib().fk_paths(ctx, n))
+    return {PATHS[k]: int(n[k]) for k in range(len(PATHS))}
 
 
 def fk_peak_fp64(device=0, stream=0, iters=1 << 15):

@@ -51,8 +51,11 @@ struct fk_ctx {
                       {nullptr, nullptr, nullptr, nullptr, nullptr}};
   cudaStream_t side = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_coef = nullptr;
+  cudaEvent_t ev_status = nullptr;     // recorded behind every queued refresh of h_status
+  bool status_pending = false;         // ... one such refresh may still be in flight
   unsigned long long* d_work = nullptr; // [N][4] per step: rows / sum prod D_k, near and other (fk_assemble)
   double class_updates[FK_K_COUNT] = {0, 0, 0, 0, 0, 0, 0};   // node-step updates per kernel class
+  unsigned long long* d_paths = nullptr; // FK_FLAG_COUNT_PATHS: FK_PATH_COUNT counters (== g.paths)
   int* d_status = nullptr;             // device status word: FK_BAD_* bits raised by fk_assemble
   int* h_status = nullptr;             // pinned host copy, refreshed at the end of every fk_evolve
   int* d_far = nullptr;                // [slots] rows per loaded step that leave the fused halo
@@ -173,6 +176,7 @@ void release(fk_ctx* c) {
     if (c->ev_free[i]) cudaEventDestroy(c->ev_free[i]);
   }
   if (c->ev_coef) cudaEventDestroy(c->ev_coef);
+  if (c->ev_status) cudaEventDestroy(c->ev_status);
   if (c->side) cudaStreamDestroy(c->side);
   cudaFree(c->opb.w);
   cudaFree(c->opb.off);
@@ -182,6 +186,7 @@ void release(fk_ctx* c) {
   cudaFree(c->d_far_line);
   cudaFree(c->d_work);
   cudaFree(c->d_status);
+  cudaFree(c->d_paths);
   if (c->h_status) cudaFreeHost(c->h_status);
   cudaFree(c->d_stage);
   for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -247,7 +252,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   if (cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, p->device) != cudaSuccess ||
       cc_major != 10)
     return fail(nullptr, FK_ECUDA, "device is not compute capability 10.x: the kernels are built for sm_100a only");
-  if (p->flags & ~(unsigned)(FK_FLAG_VALIDATE | FK_FLAG_WEIGHTED_SLOPES | FK_FLAG_MULTISTEP))
+  if (p->flags & ~(unsigned)(FK_FLAG_VALIDATE | FK_FLAG_WEIGHTED_SLOPES | FK_FLAG_MULTISTEP | FK_FLAG_COUNT_PATHS))
     return fail(nullptr, FK_EINVAL, "unknown bits in flags");
   const int shard_count = p->shard_count <= 0 ? 1 : p->shard_count;
   if (p->shard_index < 0 || p->shard_index >= shard_count)
@@ -276,6 +281,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   g.sq = std::sqrt(2.0 * p->dt);
   g.validate = (p->flags & FK_FLAG_VALIDATE) ? 1 : 0;
   g.weighted = (p->flags & FK_FLAG_WEIGHTED_SLOPES) ? 1 : 0;
+  g.paths = nullptr;
   g.shard_index = p->shard_index;
   g.shard_count = shard_count;
   g.near_lo = 0;
@@ -375,6 +381,7 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   FK_CREATE_CUDA(cudaMalloc(&c->d_coef, sizeof(double) * (size_t)slots * 2 * p->d * J));
   FK_CREATE_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
   FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_coef, cudaEventDisableTiming));
+  FK_CREATE_CUDA(cudaEventCreateWithFlags(&c->ev_status, cudaEventDisableTiming));
   for (int i = 0; i < 2; ++i) {
     FK_CREATE_CUDA(cudaMalloc(&c->op[i].w, sizeof(double2) * (size_t)J * g.RS));
     FK_CREATE_CUDA(cudaMalloc(&c->op[i].off, sizeof(int) * (size_t)J * g.RS));
@@ -385,6 +392,11 @@ int fk_create(const fk_params* p, fk_ctx** out) {
   }
   FK_CREATE_CUDA(cudaMalloc(&c->d_work, sizeof(unsigned long long) * 4 * (size_t)p->N));
   FK_CREATE_CUDA(cudaMemsetAsync(c->d_work, 0, sizeof(unsigned long long) * 4 * (size_t)p->N, c->stream));
+  if (p->flags & FK_FLAG_COUNT_PATHS) {
+    FK_CREATE_CUDA(cudaMalloc(&c->d_paths, sizeof(unsigned long long) * FK_PATH_COUNT));
+    FK_CREATE_CUDA(cudaMemsetAsync(c->d_paths, 0, sizeof(unsigned long long) * FK_PATH_COUNT, c->stream));
+    c->g.paths = c->d_paths;
+  }
   FK_CREATE_CUDA(cudaMalloc(&c->d_status, sizeof(int)));
   FK_CREATE_CUDA(cudaMemsetAsync(c->d_status, 0, sizeof(int), c->stream));
   FK_CREATE_CUDA(cudaHostAlloc(&c->h_status, sizeof(int), cudaHostAllocDefault));
@@ -438,6 +450,12 @@ int fk_reset(fk_ctx* c) {
   FK_CUDA(c, cudaMemsetAsync(c->d_status, 0, sizeof(int), c->stream));
   FK_CUDA(c, cudaMemsetAsync(c->d_work, 0, sizeof(unsigned long long) * 4 * (size_t)c->N, c->stream));
   for (int k = 0; k < FK_K_COUNT; ++k) c->class_updates[k] = 0.0;
+  // a refresh of h_status queued by the last fk_evolve may not have landed yet: wait for it, or its
+  // stale bits would overwrite the cleared word and fail the next call for no reason
+  if (c->status_pending) {
+    FK_CUDA(c, cudaEventSynchronize(c->ev_status));
+    c->status_pending = false;
+  }
   *c->h_status = 0;
   c->auto_assembled = false;           // its work counters were just cleared: assemble once more
   c->cur = 0;
@@ -451,12 +469,12 @@ int fk_set_coeffs_range(fk_ctx* c, int step0, int count, const double* b, const 
                         int mem) {
   if (!c) return FK_EINVAL;
   if (!b || !sigma) return fail(c, FK_EINVAL, "b or sigma is NULL");
-  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
+  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE && mem != FK_MEM_HOST_PINNED) return fail(c, FK_EINVAL, "bad mem kind");
   if (count < 1 || count > c->slots) return fail(c, FK_EINVAL, "count must be 1..coeff_slots");
   if (step0 < 0 || step0 + count > c->N) return fail(c, FK_EINVAL, "step range outside 0..N-1");
   DeviceGuard guard(c->device);
   const size_t slice = (size_t)c->g.d * c->g.J;      // doubles per [d][J] array
-  const cudaMemcpyKind kind = mem == FK_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  const cudaMemcpyKind kind = mem == FK_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   for (int i = 0; i < count; ++i) {
     const int step = step0 + i, slot = step % c->slots;
     double* dst = c->d_coef + (size_t)slot * 2 * slice;
@@ -487,10 +505,10 @@ int fk_set_coeffs(fk_ctx* c, int step, const double* b, const double* sigma, int
   if (!c) return FK_EINVAL;
   if (step != FK_ALL_STEPS) return fk_set_coeffs_range(c, step, 1, b, sigma, mem);
   if (!b || !sigma) return fail(c, FK_EINVAL, "b or sigma is NULL");
-  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE) return fail(c, FK_EINVAL, "bad mem kind");
+  if (mem != FK_MEM_HOST && mem != FK_MEM_DEVICE && mem != FK_MEM_HOST_PINNED) return fail(c, FK_EINVAL, "bad mem kind");
   DeviceGuard guard(c->device);
   const size_t slice = (size_t)c->g.d * c->g.J;
-  const cudaMemcpyKind kind = mem == FK_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  const cudaMemcpyKind kind = mem == FK_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   FK_CUDA(c, cudaMemcpyAsync(c->d_coef, b, sizeof(double) * slice, kind, c->stream));
   FK_CUDA(c, cudaMemcpyAsync(c->d_coef + slice, sigma, sizeof(double) * slice, kind, c->stream));
   std::fill(c->slot_step.begin(), c->slot_step.end(), -2);
@@ -748,8 +766,11 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
       n -= count;
       c->n_next = n;
     }
-    if (n_from > n_to)
+    if (n_from > n_to) {
       FK_CUDA(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+      FK_CUDA(c, cudaEventRecord(c->ev_status, c->stream));
+      c->status_pending = true;
+    }
     return FK_OK;
   }
   for (int n = n_from; n > n_to; --n) {
@@ -762,8 +783,11 @@ int fk_evolve(fk_ctx* c, int n_from, int n_to) {
     c->cur ^= 1;
     c->n_next = n - 1;
   }
-  if (n_from > n_to)                 // refresh the host copy of the device status word
+  if (n_from > n_to) {               // refresh the host copy of the device status word
     FK_CUDA(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    FK_CUDA(c, cudaEventRecord(c->ev_status, c->stream));
+    c->status_pending = true;
+  }
   return FK_OK;
 }
 
@@ -899,6 +923,18 @@ int fk_profile_updates(fk_ctx* c, double* updates) {
   if (!c) return FK_EINVAL;
   if (!updates) return fail(c, FK_EINVAL, "updates is NULL");
   for (int k = 0; k < FK_K_COUNT; ++k) updates[k] = c->class_updates[k];
+  return FK_OK;
+}
+
+int fk_paths(fk_ctx* c, long long counts[FK_PATH_COUNT]) {
+  if (!c) return FK_EINVAL;
+  if (!counts) return fail(c, FK_EINVAL, "counts is NULL");
+  if (!c->d_paths) return fail(c, FK_ESTATE, "fk_paths needs FK_FLAG_COUNT_PATHS at fk_create");
+  DeviceGuard guard(c->device);
+  unsigned long long h[FK_PATH_COUNT];
+  FK_CUDA(c, cudaMemcpyAsync(h, c->d_paths, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  FK_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < FK_PATH_COUNT; ++k) counts[k] = (long long)h[k];
   return FK_OK;
 }
 

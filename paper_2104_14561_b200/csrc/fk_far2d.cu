@@ -92,7 +92,7 @@ fk_far2d(FkGrid g, FkOperator op, const double* __restrict__ Pold, const double*
       if (cnt[r].y > 0) {
         if (cnt[r].z) {                        // packed by fk_assemble: 1 + first node | last node << 16
           qlo = min(qlo, (cnt[r].z & 0xffff) - 1);
-          qhi = max(qhi, cnt[r].z >> 16);
+          qhi = max(qhi, (int)((unsigned)cnt[r].z >> 16));   // logical shift: last node up to 65534
         } else {
           const int* __restrict__ o = op.off + (size_t)(jb + r) * g.RS + q1;
           qlo = min(qlo, o[0] / FK_CW);
@@ -103,7 +103,7 @@ fk_far2d(FkGrid g, FkOperator op, const double* __restrict__ Pold, const double*
     }
   }
   const int width = qhi - qlo + 1;
-  bool dense = sum_d1 > 0 && width <= WMAX && n0e <= E0MAX &&
+  bool dense = sum_d1 > 0 && width > 0 && width <= WMAX && n0e <= E0MAX &&
                width * (6 * CPB + 4) < sum_d1 * (6 * CPB + 2);   // L1 wavefronts of the two paths
   if (dense) {                                   // the rows' dimension-0 entries on the same lines?
     int oref = INT_MAX;
@@ -120,6 +120,8 @@ fk_far2d(FkGrid g, FkOperator op, const double* __restrict__ Pold, const double*
     if (dense && lane < n0e) st.off0[lane] = oref;
   }
 
+  if (g.paths && lane == 0 && blockIdx.y == 0)           // FK_FLAG_COUNT_PATHS
+    atomicAdd(g.paths + (dense ? FK_PATH_2D_BANDED : FK_PATH_2D_SCATTERED), 1ULL);
   if (dense) {
     // ---- banded path
     for (int k = lane; k < WMAX * RB; k += 32) (&st.W1[0][0])[k] = make_double2(0.0, 0.0);

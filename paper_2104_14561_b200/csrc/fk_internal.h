@@ -17,6 +17,8 @@
 
 #include <cuda_runtime.h>
 
+#include "../../include/fk.h"   // FK_PATH_* (the only part of the ABI the kernels see)
+
 #define FK_CW 32          // columns per chunk = lanes per warp
 #define FK_QMAX 32        // == FK_MAX_Q of include/fk.h
 #define FK_GUARD_ROWS 8   // zeroed node rows before and after the P and dP allocations
@@ -42,6 +44,8 @@ struct FkGrid {
   int shard_index, shard_count;   // this context owns the chunks c with c % count == index
   int near_lo, near_hi;           // 2-D: only rows on the lines near_lo .. near_hi-1 may be FK_ROW_NEAR (set per
                                   // step by fk_evolve: lines where most rows are far go to fk_far2d whole)
+  unsigned long long* paths;      // device, FK_FLAG_COUNT_PATHS only (else NULL): FK_PATH_COUNT counters, one
+                                  // per group of four rows and step, of the path the group was contracted on
   const double2* wgt[3];  // device, weighted only: per node the normalised weights (omega_a, omega_b)
                           // attached to the two divided differences its slope is the mean of
   const double* x[3];     // device: node coordinates

@@ -173,8 +173,9 @@ __device__ __forceinline__ int assemble_row(const FkGrid& g, const double* __res
   // 2-D: first and last dimension-1 node of the row, packed into the unused third count (1 + first
   // in the low half, last in the high half; 0 = not recorded), so that fk_far2d knows a group's
   // union window from the counts alone
-  if (g.d == 2 && cnt[1] > 0 && g.n[1] < 65535)
-    cnt[2] = (1 + rowo[g.qoff[1]] / FK_CW) | ((rowo[g.qoff[1] + cnt[1] - 1] / FK_CW) << 16);
+  if (g.d == 2 && cnt[1] > 0 && g.n[1] < 65535)          // both halves < 2^16; packed and unpacked unsigned
+    cnt[2] = (int)((unsigned)(1 + rowo[g.qoff[1]] / FK_CW) |
+                   ((unsigned)(rowo[g.qoff[1] + cnt[1] - 1] / FK_CW) << 16));
   cnt[3] = near ? FK_ROW_NEAR : 0;
   op.c[j] = cj;
   if (rec) {

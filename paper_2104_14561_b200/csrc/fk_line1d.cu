@@ -123,6 +123,10 @@ cudaError_t fk_launch_line1d(const FkGrid& g, FkOperator op, int cg, int nsteps,
                              cudaStream_t s) {
   const unsigned blocks = (unsigned)(n_chunks * (FK_CW / cg));
   const size_t smem = fk_line1d_smem(g, cg);
+  // the shared-memory limit is an attribute of the FUNCTION, shared by every context of the process:
+  // another context with a shorter line may have lowered it since this one was created
+  const cudaError_t e = fk_line1d_setup(g, cg);
+  if (e != cudaSuccess) return e;
   if (cg == 8) fk_line1d<8><<<blocks, TH, smem, s>>>(g, op, nsteps, n_hi, autonomous, Pcur, Pother, N);
   else fk_line1d<4><<<blocks, TH, smem, s>>>(g, op, nsteps, n_hi, autonomous, Pcur, Pother, N);
   return cudaGetLastError();

@@ -18,7 +18,7 @@
 // groups that reach beyond H nodes along dimension 2 or need more than EMAX entries in
 // dimension 0 or 1 take the row-at-a-time path (fkd::contract_row) inside the same kernel.
 //
-// What bounds it (profiles/r2_rowblock3d_ncu_full.md): a node is 1 KB here (4 fields x 32
+// What bounds it (profiles/r2_cfg5_kernels_ncu_full.md): a node is 1 KB here (4 fields x 32
 // columns), so the L1 holds ~190 nodes and about half of the loads miss it; the L2 -> SM traffic
 // that results (~8 GB per chunk launch at ~4.5 TB/s) is the limiter, not DRAM, fp64 or issue.
 // One staging serves CPB = 2 chunks, and each group pulls its own rows of the plane L2PF steps
@@ -372,6 +372,9 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     __syncwarp();
   }
   ok = ok && ok2;                                        // the static-slot blocked path
+  if (g.paths && lane == 0 && blockIdx.y == 0)           // FK_FLAG_COUNT_PATHS: which path this group takes
+    atomicAdd(g.paths + (wide ? (same ? FK_PATH_3D_WIDE : FK_PATH_3D_WIDE_MERGED)
+                              : ok ? (same ? FK_PATH_3D_SAME : FK_PATH_3D_MERGED) : FK_PATH_3D_ROWWISE), 1ULL);
 
   // ---- which dimension-2 slots carry a weight in any row decides the variant of the blocked path
   unsigned tmask = 0;
@@ -399,7 +402,13 @@ fk_rowblock3d(FkGrid g, FkOperator op, const double* __restrict__ Pold,
     const void* src = lane == 4 ? (const void*)(op.w + ja * g.RS)
                     : lane == 5 ? (const void*)(op.off + ja * g.RS) : (const void*)(op.cnt + ja * 4);
     const int bytes = rows * (lane == 4 ? g.RS * 16 : lane == 5 ? g.RS * 4 : 16);
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+    // the bulk prefetch wants a 16-byte aligned start and a size that is a multiple of 16; a row of
+    // op.off is RS*4 = 8*sum(Q_k) bytes, so with an odd sum(Q_k) every other row starts 8 bytes off:
+    // start rounded down, end rounded down (both stay inside the allocation; a hint may lose a tail)
+    const unsigned long long a0 = (unsigned long long)src & ~15ull;
+    const unsigned long long a1 = ((unsigned long long)src + (unsigned long long)bytes) & ~15ull;
+    if (a1 > a0)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a0), "r"((int)(a1 - a0)) : "memory");
   }
   for (int chunk = cfirst; chunk < clast; ++chunk) {
     const int m = fkd::column_of(g, chunk, lane);

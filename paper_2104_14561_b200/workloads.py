@@ -15,6 +15,7 @@ Only numpy (and math.erf through numpy.vectorize-free formulas) is used.
 """
 from __future__ import annotations
 
+import dataclasses
 import math
 from dataclasses import dataclass, field
 from typing import Callable, Optional, Sequence, Tuple
@@ -367,6 +368,17 @@ def small(idx: int) -> Workload:
     if idx == 7:
         return runaway_3d_radial(n=(29, 19, 0), N=13, dt=120.0 / 2000, xr=radial_grid(3, 20))
     raise KeyError(idx)
+
+
+def exit_everywhere(wl: Workload) -> Workload:
+    """Copy of `wl` in which every ABSORB face is an exit face (g = 1).  The runaway configs exit
+    only at p = p_max, so for any run the oracle can afford the field is still exactly
+    0 at small p -- where the rows with the widest stencils live -- and a comparison there is 0 = 0.
+    With p = 0 (and, in 3-D, r = 1) feeding 1 as well, those rows see non-zero data after a few steps.
+    Same grid, coefficients and operators as `wl`; only chi and the absorbed constants change."""
+    vals = np.array(wl.face_value, dtype=np.float64, copy=True)
+    vals[np.asarray(wl.face_kind) == FACE_ABSORB] = 1.0
+    return dataclasses.replace(wl, name=wl.name + "_exit_everywhere", face_value=vals)
 
 
 def random_field(J: int, seed: int, lo: float = 0.0, hi: float = 1.0) -> np.ndarray:

@@ -78,6 +78,20 @@ def test_nonuniform_grids(fk, oracle_mod):
                                [[A, A], [C, C], [C, A]], [[0, 1], [0, 0], [0, 0.5]], 7))
 
 
+def test_3d_odd_quadrature_sum_and_odd_last_dimension(fk, oracle_mod):
+    """A row of the operator's offset table is 8 * sum(Q_k) bytes: with an odd sum(Q_k) every other
+    row starts 8 bytes off a 16-byte boundary, which the L2 bulk prefetch of fk_rowblock3d (rows of
+    the plane three steps ahead, so n0 > 3) must round (it needs a 16-byte aligned start and size).
+    Odd n2 as well, so that group starts jb take both parities.  Every face value non-zero."""
+    lin = lambda n: np.linspace(0.0, 1.0, n)
+    for name, n, Q, seed in (("odd555", (9, 7, 13), (5, 5, 5), 21), ("odd665", (8, 6, 65), (6, 6, 5), 22),
+                             ("odd311", (7, 5, 11), (3, 1, 1), 23)):
+        wl = make(name, [lin(n[0]), lin(n[1]), lin(n[2])], 2e-3, 9, Q, [[A, A], [C, A], [C, A]],
+                  [[0.5, 1.0], [0.0, 0.75], [0.0, 0.25]], seed, drift=1.0, sigma=0.1)
+        got = check(fk, oracle_mod, wl)
+        assert float(np.abs(got[-1].reshape(n)[1:-1, 1:-1, 1:-1]).max()) > 1e-3   # informative
+
+
 def test_2d_far_rows_only_and_mixed(fk, oracle_mod):
     lin = lambda n: np.linspace(-1.0, 1.0, n)
     # sigma sqrt(2 dt) a_max ~ 14 cells: every row leaves the 2-node halo -> generic kernels only
@@ -97,6 +111,80 @@ def test_2d_far_rows_only_and_mixed(fk, oracle_mod):
         return b, s
     wl.coeffs = coeffs
     check(fk, oracle_mod, wl)
+
+
+def test_2d_far_rows_beyond_node_32768_of_dimension_1(fk, oracle_mod):
+    """fk_assemble packs a far row's first and last dimension-1 node into one int (16 bits each): with
+    more than 32768 nodes along dimension 1 the last node reaches the sign bit and must be unpacked
+    unsigned, or fk_far2d sees an empty window and returns c_j alone.  Reach of 3-14 cells (banded and
+    scattered groups), a box so thin in dimension 0 that its faces feed every node: no 0 = 0 compare."""
+    B, solve = fk
+    n1 = 40001
+    wl = make("wide_n1", [np.linspace(0.0, 3e-4, 4), np.linspace(-1.0, 1.0, n1)], 1e-6, 3, [2, 4],
+              [[A, A], [A, A]], [[1.0, 0.5], [0.25, 1.0]], 31, drift=1.0, sigma=0.3)
+    ref = oracle_mod.Oracle(wl).algorithm1()
+    ctx = solve.create_for(wl, wl.N)
+    try:
+        B.fk_profile(ctx, True)
+        solve.evolve_loaded(ctx, wl, wl.N)
+        got = np.empty((wl.N + 1, wl.J))
+        B.fk_read(ctx, 0, wl.N + 1, got)
+        prof = B.fk_profile_read(ctx)
+    finally:
+        B.fk_destroy(ctx)
+    assert prof["far2d"][1] == wl.N, prof
+    high = ref[-1].reshape(4, n1)[1:3, 32768:-1]             # updated rows beyond node 32768
+    assert float(np.mean(np.abs(high) > 1e-3)) > 0.9         # informative
+    err = float(np.abs(got - ref).max())
+    assert err <= TOL, f"{wl.name}: max abs error {err:.3e}"
+
+
+def test_reset_straight_after_a_failed_evolve(fk):
+    """fk_reset without a sync after an fk_evolve that raised the device's error flag: the refresh
+    of the host copy queued by that fk_evolve must not land after the reset cleared it."""
+    B, solve = fk
+    wl = W.small(3)
+    b, s = wl.coeff_table(0, wl.N)
+    s_bad = s.copy()
+    s_bad[3, 0, wl.J // 2 + 1] = -0.1
+    for _ in range(3):
+        ctx = solve.create_for(wl, wl.N)
+        try:
+            B.fk_set_coeffs_range(ctx, 0, wl.N, b, s_bad)
+            B.fk_evolve(ctx, wl.N, 0)                        # queued; raises the flag on the device
+            B.fk_reset(ctx)                                  # no fk_check / sync in between
+            B.fk_set_coeffs_range(ctx, 0, wl.N, b, s)
+            B.fk_evolve(ctx, wl.N, 0)
+            B.fk_evolve(ctx, 0, 0)                           # entry check only
+            out = np.empty((1, wl.J))
+            B.fk_read(ctx, wl.N, wl.N + 1, out)
+            B.fk_check(ctx)
+        finally:
+            B.fk_destroy(ctx)
+
+
+def test_two_multistep_contexts_with_different_lines(fk, oracle_mod):
+    """fk_line1d's dynamic shared-memory limit is a per-function attribute, shared by every context:
+    a second FK_FLAG_MULTISTEP context with a shorter line must not break launches of the first."""
+    B, solve = fk
+    long_wl = W.config(2, N=40, dt=W.config(2).dt)           # J = 1025: 197 KB of shared memory
+    short_wl = W.small(1)                                    # J = 201
+    ref = oracle_mod.Oracle(long_wl).algorithm1()
+    a = solve.create_for(long_wl, long_wl.N, flags=B.FK_FLAG_MULTISTEP)
+    try:
+        b = solve.create_for(short_wl, 1, flags=B.FK_FLAG_MULTISTEP)
+        try:
+            B.fk_profile(a, True)
+            solve.evolve_loaded(b, short_wl, 1)
+            solve.evolve_loaded(a, long_wl, long_wl.N)
+            got = np.empty((long_wl.N + 1, long_wl.J))
+            B.fk_read(a, 0, long_wl.N + 1, got)
+            assert B.fk_profile_read(a)["line1d"][1] > 0
+        finally:
+            B.fk_destroy(b)
+    finally:
+        B.fk_destroy(a)
+    assert float(np.abs(got - ref).max()) <= TOL
 
 
 def test_2d_lines_handed_over_at_either_end(fk, oracle_mod):

@@ -7,14 +7,22 @@ grid for N' = m steps with the config's own dt reproduces column m of the full r
 column before it), so deep columns and prefixes are compared exactly:
 
   config 2   prefix N' = 64 (all columns 0..64) and the columns m = 125, 500, 1000 (= N)
-  config 3   column m = 250 and the deep column m = 1000 (m = 2000 = N with FK_SLOW=1)
+  config 3   columns m = 250, 1000 and 2000 (= N, the last column of the full run)
   config 4   401 x 201: prefix N' = 8 and column m = 312 (= N/16); the run must use the fused
              kernel AND the far-row kernels (the real near / far mix at small p)
   config 5   161 x 81 x 65: prefix N' = 3 (one oracle application costs ~15 s of 4 cores; the
              64-step prefix SURVEY.md section 8(d) asks for would be ~9 hours)
-  FK_SLOW=1  config 3 m = 2000 (= N), config 4 m = 1250 (= N/4), config 5 prefix 6
+  FK_SLOW=1  config 4 m = 1250 (= N/4), config 5 prefix 6
 
-The worst error of each case is printed (run with -s to see it; recorded in DESIGN.md section 4).
+What those runs do NOT show: the runaway configs (4, 5, and 7 = config 5 on the paper's radial grid)
+exit only at p = p_max, so at every depth the oracle can afford their field is still exactly 0 at
+small p -- on exactly the rows that take the kernels' special paths (fk_far2d, the merged and wide
+groups of fk_rowblock3d).  The "every face an exit" cases run the same grids, coefficients and
+operators with all ABSORB faces feeding 1 (workloads.exit_everywhere); report() prints how much of
+each comparison is informative (|ref| > 1e-6) per quarter of the p lines and the tests require at
+least 10 % in the low-p quarter, and FK_FLAG_COUNT_PATHS proves the special paths ran.
+
+The figures of each case are printed (run with -s to see them; recorded in profiles/r3_parity.md).
 """
 import os
 
@@ -59,9 +67,24 @@ def gpu_columns(fk, wl, m0, m1, want_profile=False):
         B.fk_destroy(ctx)
 
 
-def report(name, got, ref):
+def report(name, got, ref, wl=None, low_share=None):
+    """Worst absolute error, and how much of the comparison says something: the share of compared
+    elements with |ref| > 1e-6, the worst relative error over |ref| > 1e-9 and, given the workload, the
+    informative share of the last compared column per quarter of the dimension-0 lines (for the
+    runaway configs the first quarter, p < p_max/4, is where the far / wide rows live).  low_share:
+    required informative share of that first quarter."""
     err = float(np.abs(got - ref).max())
-    print(f"\nPARITY {name}: max abs error {err:.3e} (max |ref| {float(np.abs(ref).max()):.3g})")
+    big = np.abs(ref) > 1e-9
+    rel = float((np.abs(got - ref)[big] / np.abs(ref)[big]).max()) if big.any() else 0.0
+    line = (f"PARITY {name}: max abs error {err:.3e}; |ref| > 1e-6 on {float(np.mean(np.abs(ref) > 1e-6)):.3f} "
+            f"of the compared elements; worst relative error over |ref| > 1e-9: {rel:.3e}")
+    if wl is not None:
+        last = np.abs(np.asarray(ref).reshape(-1, wl.J)[-1]).reshape(wl.n[0], -1)[1:-1]
+        quarters = [float(np.mean(q > 1e-6)) for q in np.array_split(last, 4)]
+        line += "; informative share by quarter of the dimension-0 lines: " + " ".join(f"{q:.2f}" for q in quarters)
+        if low_share is not None:
+            assert quarters[0] >= low_share, f"{name}: low-p quarter informative share {quarters[0]:.3f}"
+    print("\n" + line)
     assert err <= TOL, f"{name}: max abs error {err:.3e}"
     return err
 
@@ -81,7 +104,7 @@ def test_config2_prefix64(fk, oracle_mod):
     report("cfg2 prefix 64", got, ref)
 
 
-DEEP3 = [250, 1000] + ([2000] if os.environ.get("FK_SLOW") else [])
+DEEP3 = [250, 1000, 2000]                                    # 2000 = N: the last column of the full run
 
 
 @pytest.mark.parametrize("m", DEEP3)
@@ -105,6 +128,55 @@ def test_config4_full_grid_prefix_and_deep_column(fk, oracle_mod):
     ref = oracle_mod.Oracle(wl).column_streamed(m)
     got, _ = gpu_columns(fk, wl, m, m + 1)
     report(f"cfg4 401x201 column {m}", got[0], ref)
+
+
+def test_config4_every_face_an_exit_far_rows_see_nonzero_data(fk, oracle_mod):
+    """Config 4 exits only at p = p_max: at any depth the oracle can afford its field
+    is exactly 0 for p < 33, and fk_far2d's rows (p < ~12, more than half of the headline's time) are
+    compared 0 = 0 above.  Same grid, coefficients and operators with p = 0 an exit as well
+    (workloads.exit_everywhere): prefix 8 and the deep column m = 312, informative at small p."""
+    B, solve = fk
+    wl = W.exit_everywhere(prefix_config(4, 8))
+    ref = oracle_mod.Oracle(wl).algorithm1()
+    ctx = solve.create_for(wl, wl.N, flags=B.FK_FLAG_COUNT_PATHS)
+    try:
+        B.fk_profile(ctx, True)
+        solve.evolve_loaded(ctx, wl, wl.N)
+        got = np.empty((wl.N + 1, wl.J))
+        B.fk_read(ctx, 0, wl.N + 1, got)
+        prof, paths = B.fk_profile_read(ctx), B.fk_paths(ctx)
+    finally:
+        B.fk_destroy(ctx)
+    print(f"\ncfg4 exit-everywhere prefix 8: paths {paths}")
+    assert prof["far2d"][1] == 8 and prof["fused"][1] == 8, prof
+    assert paths["2d_banded"] > 0 and paths["2d_scattered"] > 0, paths
+    report("cfg4 401x201 exit-everywhere prefix 8", got, ref, wl, low_share=0.10)
+    m = 312
+    wl = W.exit_everywhere(prefix_config(4, m))
+    ref = oracle_mod.Oracle(wl).column_streamed(m)
+    got, _ = gpu_columns(fk, wl, m, m + 1)
+    report(f"cfg4 401x201 exit-everywhere column {m}", got[0], ref, wl, low_share=0.10)
+
+
+def test_config5_and_7_every_face_an_exit(fk, oracle_mod):
+    """Configs 5 and 7 (the paper's radial grid) on their full grids with p = 0 and r = 1 exits as
+    well: the r = 1 face feeds the fine radial cells at every p, including the small p where the
+    xi-wide rows and (config 7) the dimension-2 wide window run."""
+    B, solve = fk
+    for idx, steps, want in ((5, 2, ("3d_same", "3d_merged")), (7, 2, ("3d_wide", "3d_wide_merged"))):
+        wl = W.exit_everywhere(prefix_config(idx, steps))
+        ref = oracle_mod.Oracle(wl).algorithm1()
+        ctx = solve.create_for(wl, wl.N, flags=B.FK_FLAG_COUNT_PATHS)
+        try:
+            solve.evolve_loaded(ctx, wl, wl.N)
+            got = np.empty((wl.N + 1, wl.J))
+            B.fk_read(ctx, 0, wl.N + 1, got)
+            paths = B.fk_paths(ctx)
+        finally:
+            B.fk_destroy(ctx)
+        print(f"\ncfg{idx} exit-everywhere prefix {steps}: paths {paths}")
+        assert paths[want[0]] + paths[want[1]] > 0, paths
+        report(f"cfg{idx} {'x'.join(map(str, wl.n))} exit-everywhere prefix {steps}", got, ref, wl, low_share=0.10)
 
 
 @pytest.mark.skipif(not os.environ.get("FK_SLOW"), reason="minutes of oracle time: FK_SLOW=1 (run once per round, profiles/r2_parity_fullsize.md)")

@@ -114,6 +114,90 @@ def test_weighted_harmonic_mean_on_nonuniform_grids(fk, oracle_mod):
     check(fk, oracle_mod, W.small(7), "cfg7 reduced")
 
 
+def run_counted(fk, oracle_mod, wl, name):
+    """Evolve with FK_FLAG_COUNT_PATHS; -> (result, oracle, path counts).  Parity asserted."""
+    B, solve = fk
+    ref = oracle_mod.Oracle(wl).algorithm1()
+    ctx = solve.create_for(wl, wl.N, flags=B.FK_FLAG_COUNT_PATHS)
+    try:
+        solve.evolve_loaded(ctx, wl, wl.N)
+        got = np.empty((wl.N + 1, wl.J))
+        B.fk_read(ctx, 0, wl.N + 1, got)
+        paths = B.fk_paths(ctx)
+    finally:
+        B.fk_destroy(ctx)
+    err = float(np.abs(got - ref).max())
+    inner = np.abs(ref[-1].reshape(wl.n)[tuple(slice(1, -1) for _ in wl.n)])
+    share = float(np.mean(inner > 1e-6))
+    print(f"\nPARITY {name}: max abs error {err:.3e}; interior nodes of column N with |ref| > 1e-6: "
+          f"{share:.2f}; paths {paths}")
+    assert err <= TOL, f"{name}: {err:.3e}"
+    assert share >= 0.5, f"{name}: only {share:.2f} of the interior is informative"
+    return got, ref, paths
+
+
+def scaled_sigma(wl, k, factor):
+    base = wl.coeffs
+
+    def coeffs(n):
+        b, s = base(n)
+        s = s.copy()
+        s[k] = s[k] * factor
+        return b, s
+    wl.coeffs = coeffs
+    return wl
+
+
+def test_3d_wide_rows_along_a_fine_last_dimension(fk, oracle_mod):
+    """fk_rowblock3d<1>::contract_wide on NON-ZERO data: a fine non-uniform last dimension (the
+    paper's radial grid shape: coarse spacing 0.233, fine 0.0075) with a dimension-2
+    spread of 3-12 fine cells, every face an exit with its own value, so the whole interior is
+    informative after a few steps.  (a) small drift: the four rows of a group put their dimension-0 / 1
+    entries on the same nodes -> the wide window alone; (b) strong random drift in dimension 0 / 1: the
+    rows of a group land in different cells -> list merge AND wide window together.  The path counters
+    prove which paths ran."""
+    xr = W.radial_grid(3, 40)                               # 44 nodes
+    lin = lambda n: np.linspace(0.0, 1.0, n)
+    vals = [[1.0, 0.5], [0.75, 0.25], [0.6, 0.9]]
+    kinds = [[A, A], [A, A], [A, A]]
+    wl = scaled_sigma(rnd("wide3d_same", [lin(9), lin(7), xr], 1e-3, 6, [3, 3, 4], kinds, vals, 51,
+                          drift=0.02, sigma=0.3, slope_rule=1), 2, 4.0)
+    # identical dimension-0 / 1 coefficients along dimension 2: the four rows of a group agree there
+    base_same = wl.coeffs
+
+    def coeffs_same(n):
+        b, s = base_same(n)
+        b, s = b.copy().reshape(3, 9, 7, 44), s.copy().reshape(3, 9, 7, 44)
+        for a in (b, s):
+            a[0] = a[0][:, :, :1]
+            a[1] = a[1][:, :, :1]
+        return b.reshape(3, -1), s.reshape(3, -1)
+    wl.coeffs = coeffs_same
+    _, _, paths = run_counted(fk, oracle_mod, wl, "3-D wide window, rows agree in dimension 0 / 1")
+    assert paths["3d_wide"] > 0, paths
+    wl = scaled_sigma(rnd("wide3d_merge", [lin(9), lin(7), xr], 1e-3, 6, [3, 3, 4], kinds, vals, 52,
+                          drift=60.0, sigma=0.3, slope_rule=0), 2, 4.0)
+    _, _, paths = run_counted(fk, oracle_mod, wl, "3-D wide window + merged lists")
+    assert paths["3d_wide_merged"] > 0, paths
+
+
+def test_more_than_eight_quadrature_points_per_dimension(fk, oracle_mod):
+    """fk.h allows Q up to 32; the blocked kernels stage at most 16 entries per dimension.  2-D far
+    rows with Q = (12, 12) and a spread over many cells (more than 16 distinct lines in dimension 0:
+    fk_far2d's scattered path), 3-D with Q = (9, 9, 9) and a spread that gives more than 16 distinct
+    nodes in dimension 0 / 1 (fk_rowblock3d falls back to one row at a time).  Every face an exit."""
+    lin = lambda n: np.linspace(0.0, 1.0, n)
+    wl = rnd("q12_2d", [lin(61), lin(53)], 5e-3, 5, [12, 12], [[A, A], [A, A]], [[1.0, 0.5], [0.75, 0.25]],
+             53, drift=0.5, sigma=0.9)
+    _, _, paths = run_counted(fk, oracle_mod, wl, "2-D far rows, Q = (12, 12)")
+    assert paths["2d_scattered"] > 0, paths
+    wl = rnd("q9_3d", [lin(41), lin(37), lin(9)], 5e-3, 4, [9, 9, 9], [[A, A], [A, A], [A, A]],
+             [[1.0, 0.5], [0.75, 0.25], [0.6, 0.9]], 54, drift=0.5, sigma=0.9)
+    wl = scaled_sigma(wl, 2, 0.05)                          # dimension 2 stays within two nodes
+    _, _, paths = run_counted(fk, oracle_mod, wl, "3-D, Q = (9, 9, 9), long lists in dimension 0 / 1")
+    assert paths["3d_rowwise"] > 0, paths
+
+
 def test_runaway_on_the_papers_radial_grid_full_size(fk, oracle_mod):
     """161 x 81 x 128 nodes, spacing 0.1 / 0.0025 in r, weighted slopes: prefix 2."""
     full = W.config(7)

@@ -48,6 +48,43 @@ def test_small_config_matches_oracle(fk, oracle_P, idx):
     assert np.array_equal(got[0], ref[0])
 
 
+def _exit_everywhere_small(idx):
+    if idx == 4:
+        return W.exit_everywhere(W.small(4))
+    if idx == 5:
+        return W.exit_everywhere(W.runaway_3d(n=(37, 23, 19), N=10, dt=120.0 / 2000))
+    return W.exit_everywhere(W.runaway_3d_radial(n=(29, 19, 0), N=8, dt=120.0 / 2000, xr=W.radial_grid(3, 20)))
+
+
+@pytest.mark.parametrize("idx", [4, 5, 7])
+def test_small_runaway_configs_with_every_face_an_exit(fk, oracle_mod, idx):
+    """The runaway configs exit only at p = p_max: in the run above their field is
+    still exactly 0 at small p, where the rows with the widest stencils are, so those rows are compared
+    0 = 0.  Same operators with every ABSORB face feeding 1 (workloads.exit_everywhere): the low-p
+    quarter of the grid now holds non-zero values, and the kernels' special-cased paths are counted."""
+    B, solve = fk
+    wl = _exit_everywhere_small(idx)
+    ref = oracle_mod.Oracle(wl).algorithm1()
+    ctx = solve.create_for(wl, wl.N, flags=B.FK_FLAG_COUNT_PATHS)
+    try:
+        solve.evolve_loaded(ctx, wl, wl.N)
+        got = np.empty((wl.N + 1, wl.J))
+        B.fk_read(ctx, 0, wl.N + 1, got)
+        paths = B.fk_paths(ctx)
+    finally:
+        B.fk_destroy(ctx)
+    err = float(np.abs(got - ref).max())
+    low_p = np.abs(ref[-1].reshape(wl.n)[1:max(2, wl.n[0] // 4)])
+    share = float(np.mean(low_p > 1e-6))
+    print(f"\nPARITY {wl.name}: max abs error {err:.3e}; informative share at low p {share:.2f}; paths {paths}")
+    assert err <= TOL, f"{wl.name}: max abs error {err:.3e}"
+    assert share >= 0.10, share
+    if idx == 4:
+        assert paths["2d_banded"] > 0 and paths["2d_scattered"] > 0, paths
+    else:                                   # these reduced shapes stay on the static-slot path; the merged, wide
+        assert paths["3d_same"] > 0, paths  # and row-at-a-time paths are counted in tests/test_gpu_next.py
+
+
 @pytest.mark.parametrize("idx", [1, 2])
 def test_1d_stepwise_and_multistep_paths(fk, oracle_P, idx):
     """1-D problems run through the generic slopes / apply kernels by default and through fk_line1d
@@ -93,6 +130,30 @@ def test_coefficient_ring_equals_full_table(fk, oracle_P, idx, slots):
     wl, ref = oracle_P(idx)
     got = solve.evolve(wl, coeff_slots=slots)
     assert np.abs(got - ref).max() <= TOL
+
+
+@pytest.mark.parametrize("idx,slots", [(2, 7), (3, 5), (5, 4)])
+def test_ring_fed_from_pinned_host_memory_without_waiting(fk, oracle_P, idx, slots):
+    """FK_MEM_HOST_PINNED: the ring pieces are queued from page-locked host memory and the calls do
+    not synchronise, so every upload is ordered only by the stream against the kernels that still
+    read the slots it overwrites (the side stream's assemblies included).  Same result as the full
+    table, and as the oracle."""
+    import torch
+    B, solve = fk
+    wl, ref = oracle_P(idx)
+    b, s = wl.coeff_table(0, wl.N)
+    hb, hs = torch.from_numpy(b).pin_memory(), torch.from_numpy(s).pin_memory()
+    ctx = solve.create_for(wl, slots)
+    try:
+        solve.evolve_loaded(ctx, wl, slots, table=(hb, hs), pinned_async=True)
+        got = np.empty((wl.N + 1, wl.J))
+        B.fk_read(ctx, 0, wl.N + 1, got)
+    finally:
+        B.fk_destroy(ctx)
+    assert np.abs(got - ref).max() <= TOL
+    assert np.array_equal(got, solve.evolve(wl))            # bit for bit the full-table run
+    with pytest.raises(ValueError):
+        B.fk_set_coeffs_range(None, 0, 1, b[:1], s[:1], pinned_async=True)   # pageable numpy: refused by the binding
 
 
 def test_read_subrange_and_device_destination(fk, oracle_P):

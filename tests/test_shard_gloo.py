@@ -1,5 +1,9 @@
-"""Column sharding across ranks needs no data-path collective: the host-side ownership rule,
-exercised under torch.distributed (gloo, world_size 2) on CPU."""
+"""The column-ownership RULE only (solve.owned_columns), under torch.distributed (gloo, world_size 2)
+on CPU: every column has exactly one owner and round-robin chunks balance the triangular work.  No
+fk context is created here (there is no GPU on the CPU box): that fk_params.shard_* contexts
+reproduce the unsharded run bit for bit, with no exchange, is checked on the GPU by
+tests/test_gpu_next.py::test_column_shards_reproduce_the_unsharded_run (one process, every shard
+in turn) and, for the reductions, by tests/test_zz_no_alloc.py."""
 import os
 import socket
 import sys
